@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py -- grind time of one SSP-RK3 step of the 3D IGR Euler hot path on B200.
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload jets33_1024]
+                    [--storage f32|f16|bf16] [--fused 0|1]
+
+A "step" is one pass of the whole hot path (halo/BC, source, Jacobi, RHS, RK update, x3 stages) over
+the synthetic many-jet workload (config 5 of BASELINE.json at N=1).  Prints ONE JSON line.
+metric = grind time ns/(cell*eqn*RHS) = t_step / (cells * 5 * 3); lower is better.
+Multi-GPU: the path's halo exchange is not built yet, so --gpus N runs N independent
+replicas ("replicas only"): value = time / (total cells * 15), max over ranks.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "grind time ns/(cell*eqn*RHS), 3D IGR Euler SSP-RK3 step"
+UNIT = "ns/(cell*eqn*RHS)"
+# algorithmic HBM bytes per cell per launch of each row, fp32 storage
+ALG_BYTES_F32 = {"sigma_source": 20.0, "jacobi": 16.0, "rhs": 44.0, "rk_update": 73.3}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="jets33_1024")
+    ap.add_argument("--storage", default="f32", choices=["f32", "f16", "bf16"])
+    ap.add_argument("--fused", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def make_workload(name):
+    from paper_2505_07392_b200 import workloads as W
+    kind, n = name.rsplit("_", 1)
+    n = int(n)
+    if kind == "jets33":
+        scale = n / 1024.0
+        if n >= 1024:
+            return W.jets33(n=n)
+        rings = tuple((max(2, round(R * scale * 2)), c) for R, c in ((14, 3), (44, 10), (84, 20)))
+        return W.jets33(n=n, radius=max(4, round(8 * max(scale * 2, 0.5))), rings=rings)
+    if kind == "jets9":
+        return W.jets9(n=n) if n >= 512 else W.jets9(n=n, radius=max(4, n // 50), pitch=max(16, n // 8))
+    if kind == "taylor_green":
+        return W.taylor_green(n)
+    raise SystemExit("unknown workload " + name)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm = sorted(int(float(r[0])) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        mx = [int(float(r[1])) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def cpu_baseline(w, n_box=96, steps=2):
+    """The oracle, as it stands, on a bounded sample of the same workload: an n_box^3 sub-box on the
+    inflow plane around the first jet, `steps` steps, all host cores (OpenMP)."""
+    import numpy as np
+    from paper_2505_07392_b200 import workloads as W
+    cores = len(os.sched_getaffinity(0))
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    from oracle import igr_ref as R
+    if w.kind == "jets":
+        cx, cy, _ = w.params["jet_centers"][0]
+        lo = [int(max(0, min(w.nx - n_box, cx - n_box // 2))), int(max(0, min(w.ny - n_box, cy - n_box // 2))), 0]
+        nb = min(n_box, w.nx)
+        wb = W.subbox(w, tuple(lo), (lo[0] + nb, lo[1] + nb, nb))
+    else:
+        wb = type(w)(**{**w.__dict__, "nx": min(n_box, w.nx), "ny": min(n_box, w.ny), "nz": min(n_box, w.nz)})
+    q = W.state(wb).numpy().astype(np.float64)
+    s = R.RefSolver(wb.nx, wb.ny, wb.nz, wb.dx, wb.gamma, wb.alpha, order=wb.order, n_jacobi=wb.n_jacobi,
+                    faces=wb.faces, patches=wb.patches)
+    s.set_state(q)
+    dt = wb.cfl * wb.dx / s.max_wavespeed()
+    s.step(dt)                                   # untimed first touch
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        s.step(wb.cfl * wb.dx / s.max_wavespeed())
+    dt_wall = time.perf_counter() - t0
+    cells = wb.nx * wb.ny * wb.nz
+    return {"value": dt_wall / steps / (cells * 15) * 1e9, "unit": UNIT, "cores": int(os.environ["OMP_NUM_THREADS"]),
+            "kind": "oracle", "sample": "%dx%dx%d sub-box of %s on the inflow plane, %d steps, fp64, OpenMP"
+            % (wb.nx, wb.ny, wb.nz, w.name, steps), "ms_per_step": dt_wall / steps * 1e3}
+
+
+def alg_bytes(row, storage):
+    """Algorithmic HBM bytes per cell per launch: q and Sigma in the storage
+    type (s bytes), b and r in fp32.  source: 4 q reads + b write; jacobi (5 sweeps blocked, ideal):
+    rho + b + Sigma in + Sigma out; rhs: 5 q + Sigma reads + 5 r writes; rk_update: averaged over the
+    3 stages (q_n, q_s reads except stage 1, r read, q write)."""
+    s = 4 if storage == "f32" else 2
+    return {"sigma_source": 4 * s + 4, "jacobi": 3 * s + 4, "rhs": 6 * s + 20,
+            "rk_update": (5 * (s + 4 + s) + 2 * 5 * (2 * s + 4 + s)) / 3.0}[row]
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2505_07392_b200 import igr, workloads as W
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    w = make_workload(args.workload)
+    storage = {"f32": igr.STORE_F32, "f16": igr.STORE_F16, "bf16": igr.STORE_BF16}[args.storage]
+    g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
+    q0 = W.state(w, device=dev)
+    g.set_state(q0)
+    g.sync()
+    cells = w.n_cells
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step():
+        g.step(w.cfl * w.dx / g.max_wavespeed())
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = g.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    for _ in range(args.steps):
+        one_step()
+    e1.record(g.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.kernel_launches() - l0
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / args.steps
+    grind = ms_step * 1e6 / (cells * 15)             # every rank does `cells`: per-job value is the same
+
+    # per-row CUDA-event timing on the solver's stream (separate region, same state)
+    nprof = max(1, min(args.steps, 5))
+    g.profile(True)
+    for _ in range(nprof):
+        one_step()
+    rows = g.profile_read()
+    g.profile(False)
+    row_ms = {r: (v[0] / v[1] if v[1] else 0.0) for r, v in rows.items()}
+    step_ms_prof = sum(v[0] for v in rows.values()) / nprof
+    dom = max(("sigma_source", "jacobi", "rhs", "rk_update"), key=lambda r: rows[r][0])
+    peak, peak_src = measured_peaks()
+    ach = alg_bytes(dom, args.storage) * cells / (row_ms[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peak_src, "alg_bytes_per_cell": alg_bytes(dom, args.storage),
+                "avg_launch_ms": row_ms[dom], "share_of_step": rows[dom][0] / nprof / step_ms_prof,
+                "rows_ms_per_call": row_ms,
+                "rows_frac_of_peak": {r: alg_bytes(r, args.storage) * cells / (row_ms[r] * 1e-3) / 1e9 / peak
+                                      for r in ("sigma_source", "jacobi", "rhs", "rk_update") if row_ms[r] > 0},
+                "step_hbm_frac_of_peak": (3 * (alg_bytes("sigma_source", args.storage) + alg_bytes("jacobi", args.storage)
+                                               + alg_bytes("rhs", args.storage) + alg_bytes("rk_update", args.storage))
+                                          * cells / (ms_step * 1e-3) / 1e9 / peak)}
+
+    # end to end through the C ABI with HOST buffers: set_state (H2D) + wave speed + step + get_state (D2H)
+    e2e = None
+    if args.e2e_steps > 0:
+        del q0
+        torch.cuda.empty_cache()
+        try:
+            host = torch.empty((5, w.nz, w.ny, w.nx), dtype=torch.float32, pin_memory=True)
+            pinned = True
+        except RuntimeError:
+            host = torch.empty((5, w.nz, w.ny, w.nx), dtype=torch.float32)
+            pinned = False
+        g.get_state(host)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            g.set_state(host)
+            g.step(w.cfl * w.dx / g.max_wavespeed())
+            g.get_state(host)
+        barrier()
+        t_e2e = (time.perf_counter() - t0) / args.e2e_steps
+        if world > 1:
+            t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        nbytes = 5 * cells * 4
+        e2e = {"value": t_e2e * 1e9 / (cells * 15), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes + 8, "ms_per_step": t_e2e * 1e3, "pinned_host": pinned}
+
+    out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
+                      "storage": args.storage, "fused": args.fused, "n_jacobi": w.n_jacobi, "order": w.order,
+                      "cfl": w.cfl, "parallelism": "replicas only" if world > 1 else "single GPU",
+                      "l2": "inputs larger than L2 (no flush needed)" if cells * 4 > (126 << 20) else "inputs fit L2",
+                      "wavespeed_query_every_step": True},
+           "cell_updates_per_s": world * cells / (ms_step * 1e-3),
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(w)
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    w = make_workload(args.workload)
+    steps = max(1, min(args.steps, 3))
+    cb = cpu_baseline(w, n_box=96, steps=steps)
+    out = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
+           "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": steps, "warmup": 1,
+           "ms_per_step": cb["ms_per_step"], "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "sample": cb["sample"]},
+           "cpu_baseline": {"value": cb["value"], "unit": UNIT, "kind": "oracle", "cores": cb["cores"],
+                            "sample": cb["sample"]},
+           "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -1,0 +1,146 @@
+/* igr.h -- C ABI of libigr.so: one SSP-RK3 time step of the 3D compressible Euler equations with
+ * information geometric regularisation (IGR) on one NVIDIA B200 (sm_100a).
+ *
+ * Source of every operation: arXiv 2505.07392 as extracted in PAPER.md (cited "L<line>"), read as
+ * recorded in DESIGN.md ("Readings", A1-A18).  The library is hand-written CUDA; there is no CPU
+ * fallback: every call fails with IGR_ERR_CUDA if no usable device is present.
+ *
+ * The method (section 4.1; Algorithm 1):
+ *   state q = (rho, m_x, m_y, m_z, E) on a uniform Cartesian grid of nx*ny*nz cells of size dx;
+ *   entropic pressure Sigma from   Sigma/rho - alpha div(grad(Sigma)/rho) = alpha (tr((grad u)^2) + (tr grad u)^2)
+ *   (eq. 9) by n_jacobi warm-started Jacobi sweeps of the 6-point stencil (L130, L138);
+ *   fluxes with p + Sigma (eqs. 6-8), 5th-order linear reconstruction of the conserved
+ *   variables and Sigma, Lax-Friedrichs flux (L132, Alg. 1); SSP-RK3 in time (L138).
+ *
+ * Conventions
+ *   - All functions return 0 (IGR_OK) or a negative igr_status; nothing throws or aborts.
+ *   - Field layout at the boundary: interior cells only, x fastest: q[c][k][j][i] with c = 0..4,
+ *     i.e. index ((c*nz + k)*ny + j)*nx + i; always fp32, also in reduced-storage mode.
+ *   - Every `q`/`f` pointer may be a HOST or a DEVICE pointer (resolved with
+ *     cudaPointerGetAttributes); it is borrowed for the duration of the call only.
+ *   - The solver owns its device buffers (or carves them from igr_options.workspace); `bc` and the
+ *     patch arrays are copied at creation.
+ *   - igr_step and the per-kernel entry points are asynchronous on the solver's stream; CUDA errors
+ *     and non-finite states surface at the next synchronising call (igr_max_wavespeed,
+ *     igr_get_*, igr_sync).
+ */
+#ifndef IGR_H
+#define IGR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    IGR_OK = 0,
+    IGR_ERR_ARG = -1,        /* null pointer, non-positive size, gamma <= 1, order not in {3,5}, ... */
+    IGR_ERR_BC = -2,         /* periodic on only one face of an axis, unknown face code            */
+    IGR_ERR_ALLOC = -3,      /* device allocation failed or workspace too small                    */
+    IGR_ERR_CUDA = -4,       /* no device, launch or copy failure (see igr_last_error)             */
+    IGR_ERR_NONFINITE = -5   /* the state contains NaN/Inf (reported, never repaired: reading A10) */
+} igr_status;
+
+/* boundary codes per face (the paper gives no boundary conditions; BASELINE.json names these three;
+ * DESIGN.md reading A8).  Order of faces: x-, x+, y-, y+, z-, z+. */
+#define IGR_BC_PERIODIC 0    /* wrap modulo n; must be set on both faces of the axis               */
+#define IGR_BC_EXTRAP   1    /* zeroth-order extrapolation (clamp to the nearest interior cell)    */
+#define IGR_BC_INFLOW   2    /* fixed-state circular patches, extrapolation outside them           */
+
+/* storage precision of q and Sigma in device memory; arithmetic is always fp32 */
+#define IGR_STORE_F32  0
+#define IGR_STORE_F16  1
+#define IGR_STORE_BF16 2
+
+/* A circular inflow patch on a face.  (c0, c1) and radius are in CELL units on the face plane, the
+ * transverse axes taken in the order x < y < z.  A ghost cell whose transverse centre (i+1/2, j+1/2)
+ * lies at distance r from the centre gets, in all three ghost layers,
+ *     q_ghost = q_clamp + w(r) (q_fixed - q_clamp),
+ *     w = 1 for r <= radius, 0 otherwise                                   if edge == 0,
+ *     w = (1 - tanh((r - radius)/edge))/2, and exactly 0 for r >= radius + 4 edge   if edge > 0,
+ * q_fixed = (rho, rho u, rho v, rho w, p/(gamma-1) + rho |u|^2/2), q_clamp = nearest interior cell.
+ * Where several patches overlap the one with the largest w wins. */
+typedef struct {
+    double c0, c1, radius, edge;
+    double rho, u, v, w, p;
+} igr_patch;
+
+typedef struct {
+    int32_t face[6];              /* IGR_BC_* per face                                            */
+    int32_t n_patches[6];         /* used where face[f] == IGR_BC_INFLOW                          */
+    const igr_patch *patches[6];  /* host arrays, copied by igr_create                            */
+} igr_bc;
+
+typedef struct {
+    int32_t storage;       /* IGR_STORE_*                                                         */
+    int32_t fused;         /* 0: one kernel per row of the hot path (source, Jacobi, RHS, update)  */
+                           /* 1: RK update fused into the RHS kernel (one more state buffer)       */
+    void   *stream;        /* cudaStream_t to run on (NULL: the legacy default stream)             */
+    void   *workspace;     /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-B     */
+    size_t  workspace_bytes; /* aligned, at least igr_workspace_bytes(); NULL: library allocates  */
+} igr_options;
+
+typedef struct igr_solver igr_solver;
+
+/* Device bytes a solver of this size needs (for igr_options.workspace). */
+size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt);
+
+/* Create a solver.  dx: uniform spacing in all directions; gamma > 1: ideal-gas exponent (eq. 4);
+ * alpha >= 0: IGR strength, shock width ~ sqrt(alpha) (L130; the configs use 10 dx^2);
+ * order: 5 (L132) or 3; n_jacobi >= 0 sweeps per RHS evaluation (L130 "<~ 10"; configs: 5).
+ * Errors: IGR_ERR_ARG, IGR_ERR_BC, IGR_ERR_ALLOC, IGR_ERR_CUDA.  *out is NULL on failure. */
+int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
+               int n_jacobi, const igr_bc *bc, igr_solver **out);
+int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
+                  int n_jacobi, const igr_bc *bc, const igr_options *opt, igr_solver **out);
+void igr_destroy(igr_solver *s);
+
+/* Copy a state in (rounding to the storage format) and reset Sigma = 0 ("Sigma = 0 at t = 0"). */
+int igr_set_state(igr_solver *s, const float *q);
+/* Copy the current state out; synchronises.  IGR_ERR_NONFINITE is NOT raised here. */
+int igr_get_state(igr_solver *s, float *q);
+/* Sigma is part of a restart because of the warm start (L130, L138).  f: [nz][ny][nx]. */
+int igr_set_sigma(igr_solver *s, const float *f);
+int igr_get_sigma(igr_solver *s, float *f);
+
+/* max over cells of max(|u|,|v|,|w|) + sqrt(gamma p / rho): the CFL wave speed (reading A9);
+ * the caller chooses dt = CFL dx / *out.  Blocking.  IGR_ERR_NONFINITE if the state holds NaN/Inf
+ * or the result is not finite (negative pressure or density). */
+int igr_max_wavespeed(igr_solver *s, double *out);
+
+/* One SSP-RK3 step (L138, ref. 17): three RHS evaluations, each = halo/BC, source, n_jacobi
+ * warm-started sweeps, fused reconstruction + LF flux + divergence, then the stage update. */
+int igr_step(igr_solver *s, double dt);
+
+/* Block until the stream is idle; returns a pending CUDA error if any. */
+int igr_sync(igr_solver *s);
+const char *igr_last_error(const igr_solver *s);
+
+/* ---- the rows of the hot path as separate calls, for parity tests and
+ * profiling.  They act on the solver's CURRENT stage buffer (the state after igr_set_state).   */
+int igr_halo_bc(igr_solver *s);        /* a1: ghost layers of q (periodic / extrapolation / inflow) */
+int igr_sigma_source(igr_solver *s);   /* a2: b = alpha (tr((grad u)^2) + (tr grad u)^2), 2nd-order */
+                                       /*     central differences of u = m/rho (L127, L132)         */
+int igr_jacobi(igr_solver *s);         /* a3: n_jacobi sweeps from the stored Sigma + Sigma ghosts  */
+int igr_rhs(igr_solver *s);            /* a4: r = -div F^ (reconstruction, LF flux; L132, L183-L210)*/
+int igr_rk_update(igr_solver *s, int stage, double dt); /* a5: stage 1..3 of SSP-RK3 (unfused)     */
+int igr_get_source(igr_solver *s, float *f);            /* b,   [nz][ny][nx]                        */
+int igr_set_source(igr_solver *s, const float *f);      /* test hook: drive igr_jacobi with a given b */
+int igr_get_rhs(igr_solver *s, float *r);               /* r,   [5][nz][ny][nx]                     */
+/* padded copy (3 ghost layers each side) of component c = 0..4 of q, or Sigma for c = 5:
+ * f: [nz+6][ny+6][nx+6] */
+int igr_get_padded(igr_solver *s, int c, float *f);
+
+/* ---- measurement hooks (bench.py).  Rows: 0 halo_bc, 1 sigma_source, 2 jacobi (sweeps + Sigma
+ * ghosts), 3 rhs, 4 rk_update, 5 max_wavespeed (standalone reduction). */
+int igr_kernel_launches(igr_solver *s, long long *out);  /* kernels launched since igr_create     */
+int igr_profile(igr_solver *s, int enable);    /* start (1) / stop (0) per-row CUDA-event timing   */
+                                               /* on the solver's stream; clears earlier records   */
+int igr_profile_read(igr_solver *s, double ms[6], long long count[6]); /* summed ms, calls per row */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IGR_H */

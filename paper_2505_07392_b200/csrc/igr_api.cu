@@ -1,0 +1,539 @@
+// igr_api.cu -- the C ABI of libigr.so (include/igr.h): solver object, buffer carving, host<->device
+// marshalling and the sequencing of the kernels of one SSP-RK3 step.  No arithmetic of the method
+// is done on the host except the fp64 evaluation of the inflow blend weights at creation.
+#include "../../include/igr.h"
+#include "igr_kernels.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr size_t kStageBytes = 64u << 20;          // staging buffer for host <-> device copies
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline size_t elem_size(int storage) { return storage == IGR_STORE_F32 ? 4 : 2; }
+
+Grid make_grid(int nx, int ny, int nz, int storage, const int32_t *faces)
+{
+    Grid g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    const int per32 = (int)(32 / elem_size(storage));     // elements per 32 bytes
+    g.gx = per32;                                         // 8 (fp32) or 16 (half): >= 3 ghosts
+    g.px = (int)align_up((size_t)nx + 2 * g.gx, per32);
+    g.py = ny + 2 * IGR_NG;
+    g.pz = nz + 2 * IGR_NG;
+    g.sy = g.px;
+    g.sz = (long long)g.px * g.py;
+    g.np = g.sz * g.pz;
+    for (int f = 0; f < 6; ++f) g.bc[f] = faces ? faces[f] : 0;
+    return g;
+}
+
+struct Layout {
+    size_t q_bytes, f_bytes;        // one padded field in storage type / in fp32
+    int n_state;                    // state buffers (2 unfused, 3 fused)
+    size_t total;
+};
+
+Layout make_layout(const Grid &g, int storage, int fused)
+{
+    Layout L;
+    L.q_bytes = align_up((size_t)g.np * elem_size(storage), kAlign);
+    L.f_bytes = align_up((size_t)g.np * 4, kAlign);
+    L.n_state = fused ? 3 : 2;
+    // states + Sigma x2 (storage type) + b + r[5] (fp32) + staging + wave result
+    L.total = (size_t)L.n_state * 5 * L.q_bytes + 2 * L.q_bytes + 6 * L.f_bytes + kStageBytes + kAlign;
+    return L;
+}
+
+}  // namespace
+
+struct igr_solver {
+    Grid g;
+    int storage = 0, fused = 0, order = 5, n_jacobi = 5;
+    double dx = 0, gamma = 0, alpha = 0;
+    cudaStream_t stream = nullptr;
+    char *base = nullptr;            // device memory (owned or caller's workspace)
+    bool owns_base = false;
+    StagePtrs st[3];                 // state buffers: st[cur] is the current stage buffer
+    int cur = 0;                     // index of the buffer holding q^n / the current state
+    void *sig[2] = { nullptr, nullptr };
+    int sig_cur = 0;
+    float *b = nullptr;
+    float *r[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
+    float *stage = nullptr;          // staging, kStageBytes
+    WaveResult *wave = nullptr;      // device
+    bool wave_valid = false;         // wave holds the wave speed of the current state
+    BcDesc bc;
+    std::vector<void *> bc_allocs;   // device arrays of the inflow faces
+    std::string err;
+    long long launches = 0;          // kernels launched so far (igr_kernel_launches)
+    bool profile = false;            // per-row CUDA-event timing (igr_profile)
+    std::vector<cudaEvent_t> ev;     // start/stop pairs
+    std::vector<int> ev_row;
+
+    int fail(int code, const char *what, cudaError_t e = cudaSuccess)
+    {
+        char buf[512];
+        if (e != cudaSuccess) snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+        else snprintf(buf, sizeof buf, "%s", what);
+        err = buf;
+        return code;
+    }
+};
+
+namespace {
+
+// fp64 evaluation of the inflow blend weight (igr.h, igr_patch; reading A8b)
+double patch_weight(const igr_patch &p, int t0, int t1)
+{
+    const double d0 = (t0 + 0.5) - p.c0, d1 = (t1 + 0.5) - p.c1;
+    const double r2 = d0 * d0 + d1 * d1;
+    if (p.edge <= 0.0) return r2 <= p.radius * p.radius ? 1.0 : 0.0;
+    const double r = std::sqrt(r2);
+    if (r >= p.radius + 4.0 * p.edge) return 0.0;
+    return 0.5 * (1.0 - std::tanh((r - p.radius) / p.edge));
+}
+
+int build_inflow(igr_solver *s, const igr_bc *bc)
+{
+    const int n[3] = { s->g.nx, s->g.ny, s->g.nz };
+    for (int f = 0; f < 6; ++f) {
+        InflowFace &F = s->bc.inflow[f];
+        F.weight = nullptr; F.fixed = nullptr; F.n0 = F.n1 = 0;
+        if (bc->face[f] != IGR_BC_INFLOW || bc->n_patches[f] <= 0) continue;
+        if (!bc->patches[f]) return s->fail(IGR_ERR_ARG, "igr_create: inflow face without patches array");
+        const int a = f / 2;
+        F.n0 = (a == 0) ? n[1] : n[0];
+        F.n1 = (a == 2) ? n[1] : n[2];
+        std::vector<float> w((size_t)F.n0 * F.n1), fx((size_t)F.n0 * F.n1 * 5, 0.f);
+        for (int t1 = 0; t1 < F.n1; ++t1)
+            for (int t0 = 0; t0 < F.n0; ++t0) {
+                double best = 0.0; const igr_patch *bp = nullptr;
+                for (int m = 0; m < bc->n_patches[f]; ++m) {
+                    double ww = patch_weight(bc->patches[f][m], t0, t1);
+                    if (ww > best) { best = ww; bp = &bc->patches[f][m]; }
+                }
+                const size_t id = (size_t)t1 * F.n0 + t0;
+                w[id] = (float)best;
+                if (best >= 1.0) w[id] = 1.0f;
+                else if (best > 0.0 && w[id] >= 1.0f) w[id] = 0.99999994f;   // keep "w < 1" in fp32
+                if (bp) {
+                    const double ke = 0.5 * bp->rho * (bp->u * bp->u + bp->v * bp->v + bp->w * bp->w);
+                    const double v[5] = { bp->rho, bp->rho * bp->u, bp->rho * bp->v, bp->rho * bp->w,
+                                          bp->p / (s->gamma - 1.0) + ke };
+                    for (int c = 0; c < 5; ++c) fx[id * 5 + c] = (float)v[c];
+                }
+            }
+        float *dw = nullptr, *dfx = nullptr;
+        if (cudaMalloc(&dw, w.size() * 4) != cudaSuccess || cudaMalloc(&dfx, fx.size() * 4) != cudaSuccess)
+            return s->fail(IGR_ERR_ALLOC, "igr_create: cudaMalloc of inflow tables failed");
+        s->bc_allocs.push_back(dw); s->bc_allocs.push_back(dfx);
+        IGR_CUDA_OK(cudaMemcpy(dw, w.data(), w.size() * 4, cudaMemcpyHostToDevice));
+        IGR_CUDA_OK(cudaMemcpy(dfx, fx.data(), fx.size() * 4, cudaMemcpyHostToDevice));
+        F.weight = dw; F.fixed = dfx;
+    }
+    return IGR_OK;
+}
+
+bool is_device_pointer(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// copy one user field (interior, fp32, host or device) into / out of a padded field
+int field_in(igr_solver *s, const float *user, void *field, int storage)
+{
+    const Grid &g = s->g;
+    if (is_device_pointer(user)) {
+        launch_unpack_field(g, storage, user, field, 0, g.nz, s->stream);
+        return IGR_OK;
+    }
+    const size_t plane = (size_t)g.nx * g.ny * 4;
+    int chunk = (int)(kStageBytes / plane);
+    if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
+    for (int k0 = 0; k0 < g.nz; k0 += chunk) {
+        const int nk = (g.nz - k0 < chunk) ? g.nz - k0 : chunk;
+        IGR_CUDA_OK(cudaMemcpyAsync(s->stage, user + (size_t)k0 * g.nx * g.ny, nk * plane,
+                                    cudaMemcpyHostToDevice, s->stream));
+        launch_unpack_field(g, storage, s->stage, field, k0, nk, s->stream);
+    }
+    return IGR_OK;
+}
+
+int field_out(igr_solver *s, const void *field, float *user, int storage)
+{
+    const Grid &g = s->g;
+    if (is_device_pointer(user)) {
+        launch_pack_field(g, storage, field, user, 0, g.nz, s->stream);
+        return IGR_OK;
+    }
+    const size_t plane = (size_t)g.nx * g.ny * 4;
+    int chunk = (int)(kStageBytes / plane);
+    if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
+    for (int k0 = 0; k0 < g.nz; k0 += chunk) {
+        const int nk = (g.nz - k0 < chunk) ? g.nz - k0 : chunk;
+        launch_pack_field(g, storage, field, s->stage, k0, nk, s->stream);
+        IGR_CUDA_OK(cudaMemcpyAsync(user + (size_t)k0 * g.nx * g.ny, s->stage, nk * plane,
+                                    cudaMemcpyDeviceToHost, s->stream));
+        IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    }
+    return IGR_OK;
+}
+
+// times one row of the hot path with a CUDA-event pair on the solver's stream when profiling is on
+struct RowTimer {
+    igr_solver *s; int row;
+    RowTimer(igr_solver *s_, int row_, int n_launch) : s(s_), row(row_)
+    {
+        s->launches += n_launch;
+        if (!s->profile) return;
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        s->ev.push_back(a); s->ev.push_back(b); s->ev_row.push_back(row);
+        cudaEventRecord(a, s->stream);
+    }
+    ~RowTimer() { if (s->profile) cudaEventRecord(s->ev.back(), s->stream); }
+};
+
+int finish(igr_solver *s, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return s->fail(IGR_ERR_CUDA, what, e);
+    return IGR_OK;
+}
+
+}  // namespace
+
+// ===================================================================================== C ABI
+extern "C" {
+
+size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return 0;
+    const int storage = opt ? opt->storage : IGR_STORE_F32;
+    const int fused = opt ? opt->fused : 0;
+    if (storage < 0 || storage > 2) return 0;
+    Grid g = make_grid(nx, ny, nz, storage, nullptr);
+    return make_layout(g, storage, fused).total;
+}
+
+int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
+               int n_jacobi, const igr_bc *bc, igr_solver **out)
+{
+    return igr_create_ex(nx, ny, nz, dx, gamma, alpha, order, n_jacobi, bc, nullptr, out);
+}
+
+int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
+                  int n_jacobi, const igr_bc *bc, const igr_options *opt, igr_solver **out)
+{
+    if (!out) return IGR_ERR_ARG;
+    *out = nullptr;
+    if (!bc || nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(gamma > 1) || !(alpha >= 0) ||
+        n_jacobi < 0 || (order != 5 && order != 3))
+        return IGR_ERR_ARG;
+    const int storage = opt ? opt->storage : IGR_STORE_F32;
+    if (storage < 0 || storage > 2) return IGR_ERR_ARG;
+    for (int a = 0; a < 3; ++a) {
+        const int lo = bc->face[2 * a], hi = bc->face[2 * a + 1];
+        if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return IGR_ERR_BC;
+        if ((lo == IGR_BC_PERIODIC) != (hi == IGR_BC_PERIODIC)) return IGR_ERR_BC;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return IGR_ERR_CUDA; }
+
+    igr_solver *s = new igr_solver();
+    s->storage = storage;
+    s->fused = opt ? (opt->fused != 0) : 0;
+    s->order = order; s->n_jacobi = n_jacobi;
+    s->dx = dx; s->gamma = gamma; s->alpha = alpha;
+    s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
+    s->g = make_grid(nx, ny, nz, storage, bc->face);
+    const Layout L = make_layout(s->g, storage, s->fused);
+    if (opt && opt->workspace) {
+        if (opt->workspace_bytes < L.total || ((uintptr_t)opt->workspace % kAlign) != 0) {
+            delete s;
+            return IGR_ERR_ALLOC;
+        }
+        s->base = (char *)opt->workspace;
+    } else {
+        if (cudaMalloc((void **)&s->base, L.total) != cudaSuccess) {
+            cudaGetLastError();
+            delete s;
+            return IGR_ERR_ALLOC;
+        }
+        s->owns_base = true;
+    }
+    // ghosts and the x padding must hold finite numbers: zero everything once
+    if (cudaMemsetAsync(s->base, 0, L.total, s->stream) != cudaSuccess) { igr_destroy(s); return IGR_ERR_CUDA; }
+    char *p = s->base;
+    for (int b = 0; b < L.n_state; ++b)
+        for (int c = 0; c < 5; ++c) { s->st[b].f[c] = p; p += L.q_bytes; }
+    if (L.n_state < 3) s->st[2] = s->st[1];
+    s->sig[0] = p; p += L.q_bytes;
+    s->sig[1] = p; p += L.q_bytes;
+    s->b = (float *)p; p += L.f_bytes;
+    for (int c = 0; c < 5; ++c) { s->r[c] = (float *)p; p += L.f_bytes; }
+    s->stage = (float *)p; p += kStageBytes;
+    s->wave = (WaveResult *)p;
+    int rc = build_inflow(s, bc);
+    if (rc != IGR_OK) { igr_destroy(s); return rc; }
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) { igr_destroy(s); return IGR_ERR_CUDA; }
+    *out = s;
+    return IGR_OK;
+}
+
+void igr_destroy(igr_solver *s)
+{
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    for (void *p : s->bc_allocs) cudaFree(p);
+    if (s->owns_base && s->base) cudaFree(s->base);
+    delete s;
+}
+
+const char *igr_last_error(const igr_solver *s) { return s ? s->err.c_str() : "null solver"; }
+
+int igr_sync(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    return finish(s, "igr_sync");
+}
+
+int igr_set_state(igr_solver *s, const float *q)
+{
+    if (!s || !q) return IGR_ERR_ARG;
+    const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
+    s->cur = 0;
+    for (int c = 0; c < 5; ++c) {
+        int rc = field_in(s, q + c * n, s->st[0].f[c], s->storage);
+        if (rc != IGR_OK) return rc;
+    }
+    const size_t qb = (size_t)s->g.np * elem_size(s->storage);
+    IGR_CUDA_OK(cudaMemsetAsync(s->sig[0], 0, qb, s->stream));     // "Sigma = 0 at t = 0"
+    IGR_CUDA_OK(cudaMemsetAsync(s->sig[1], 0, qb, s->stream));
+    s->sig_cur = 0;
+    s->wave_valid = false;
+    return finish(s, "igr_set_state");
+}
+
+int igr_get_state(igr_solver *s, float *q)
+{
+    if (!s || !q) return IGR_ERR_ARG;
+    const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
+    for (int c = 0; c < 5; ++c) {
+        int rc = field_out(s, s->st[s->cur].f[c], q + c * n, s->storage);
+        if (rc != IGR_OK) return rc;
+    }
+    return igr_sync(s);
+}
+
+int igr_set_sigma(igr_solver *s, const float *f)
+{
+    if (!s || !f) return IGR_ERR_ARG;
+    int rc = field_in(s, f, s->sig[s->sig_cur], s->storage);
+    if (rc != IGR_OK) return rc;
+    launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);
+    return finish(s, "igr_set_sigma");
+}
+
+int igr_get_sigma(igr_solver *s, float *f)
+{
+    if (!s || !f) return IGR_ERR_ARG;
+    int rc = field_out(s, s->sig[s->sig_cur], f, s->storage);
+    if (rc != IGR_OK) return rc;
+    return igr_sync(s);
+}
+
+int igr_get_source(igr_solver *s, float *f)
+{
+    if (!s || !f) return IGR_ERR_ARG;
+    int rc = field_out(s, s->b, f, IGR_STORE_F32);
+    if (rc != IGR_OK) return rc;
+    return igr_sync(s);
+}
+
+int igr_set_source(igr_solver *s, const float *f)
+{
+    if (!s || !f) return IGR_ERR_ARG;
+    int rc = field_in(s, f, s->b, IGR_STORE_F32);
+    if (rc != IGR_OK) return rc;
+    return finish(s, "igr_set_source");
+}
+
+int igr_get_rhs(igr_solver *s, float *r)
+{
+    if (!s || !r) return IGR_ERR_ARG;
+    const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
+    for (int c = 0; c < 5; ++c) {
+        int rc = field_out(s, s->r[c], r + c * n, IGR_STORE_F32);
+        if (rc != IGR_OK) return rc;
+    }
+    return igr_sync(s);
+}
+
+int igr_get_padded(igr_solver *s, int c, float *f)
+{
+    if (!s || !f || c < 0 || c > 5) return IGR_ERR_ARG;
+    const Grid &g = s->g;
+    const void *field = c < 5 ? s->st[s->cur].f[c] : s->sig[s->sig_cur];
+    const size_t wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG, wz = g.nz + 2 * IGR_NG;
+    if (is_device_pointer(f)) {
+        launch_pack_padded(g, s->storage, field, f, 0, (int)wz, s->stream);
+        return igr_sync(s);
+    }
+    const size_t plane = wx * wy * 4;
+    int chunk = (int)(kStageBytes / plane);
+    if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr_get_padded: plane exceeds the staging buffer");
+    for (int k0 = 0; k0 < (int)wz; k0 += chunk) {
+        const int nk = ((int)wz - k0 < chunk) ? (int)wz - k0 : chunk;
+        launch_pack_padded(g, s->storage, field, s->stage, k0, nk, s->stream);
+        IGR_CUDA_OK(cudaMemcpyAsync(f + (size_t)k0 * wx * wy, s->stage, nk * plane,
+                                    cudaMemcpyDeviceToHost, s->stream));
+        IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    }
+    return finish(s, "igr_get_padded");
+}
+
+// ------------------------------------------------------------------------- rows of the hot path
+int igr_halo_bc(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    RowTimer t(s, 0, 1);
+    launch_halo_q(s->g, s->storage, s->st[s->cur], s->bc, s->stream);
+    return finish(s, "igr_halo_bc");
+}
+
+int igr_sigma_source(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    RowTimer t(s, 1, 1);
+    launch_source(s->g, s->storage, s->st[s->cur], s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
+                  s->stream);
+    return finish(s, "igr_sigma_source");
+}
+
+int igr_jacobi(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    const float k2 = (float)(s->alpha / (s->dx * s->dx));
+    RowTimer t(s, 2, s->n_jacobi + 1);
+    for (int it = 0; it < s->n_jacobi; ++it) {
+        launch_jacobi_sweep(s->g, s->storage, s->st[s->cur].f[0], s->b, s->sig[s->sig_cur],
+                            s->sig[1 - s->sig_cur], k2, s->stream);
+        s->sig_cur = 1 - s->sig_cur;
+    }
+    launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);
+    return finish(s, "igr_jacobi");
+}
+
+int igr_rhs(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    RowTimer t(s, 3, 1);
+    RhsParams p;
+    p.gamma = (float)s->gamma; p.inv_dx = (float)(1.0 / s->dx); p.order = s->order;
+    launch_rhs_simple(s->g, s->storage, s->st[s->cur], s->sig[s->sig_cur], s->r, p, s->stream);
+    return finish(s, "igr_rhs");
+}
+
+// Unfused buffer discipline (only the current sub-step enters the RHS; the buffer
+// with q^n is only read by the update): A = st[0] holds q^n, B = st[1] the sub-step.
+//   stage 1: B = A + dt r(A);  stage 2: B = A + 1/4((B - A) + dt r(B));  stage 3: A = A + 2/3((B - A) + dt r(B))
+int igr_rk_update(igr_solver *s, int stage, double dt)
+{
+    if (!s || stage < 1 || stage > 3) return IGR_ERR_ARG;
+    const float beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
+    StagePtrs &A = s->st[0], &B = s->st[1];
+    RowTimer t(s, 4, 1);
+    if (stage == 1) {
+        launch_rk_update(s->g, s->storage, A, A, B, s->r, beta, (float)dt, (float)s->gamma, nullptr, s->stream);
+        s->cur = 1;
+    } else if (stage == 2) {
+        launch_rk_update(s->g, s->storage, A, B, B, s->r, beta, (float)dt, (float)s->gamma, nullptr, s->stream);
+        s->cur = 1;
+    } else {
+        IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
+        launch_rk_update(s->g, s->storage, A, B, A, s->r, beta, (float)dt, (float)s->gamma, s->wave, s->stream);
+        s->cur = 0;
+        s->wave_valid = true;
+    }
+    return finish(s, "igr_rk_update");
+}
+
+int igr_step(igr_solver *s, double dt)
+{
+    if (!s) return IGR_ERR_ARG;
+    if (s->cur != 0) return s->fail(IGR_ERR_ARG, "igr_step: called in the middle of a step");
+    for (int stage = 1; stage <= 3; ++stage) {
+        int rc;
+        if ((rc = igr_halo_bc(s)) != IGR_OK) return rc;
+        if ((rc = igr_sigma_source(s)) != IGR_OK) return rc;
+        if ((rc = igr_jacobi(s)) != IGR_OK) return rc;
+        if ((rc = igr_rhs(s)) != IGR_OK) return rc;
+        if ((rc = igr_rk_update(s, stage, dt)) != IGR_OK) return rc;
+    }
+    return IGR_OK;
+}
+
+int igr_max_wavespeed(igr_solver *s, double *out)
+{
+    if (!s || !out) return IGR_ERR_ARG;
+    if (!s->wave_valid) {
+        RowTimer t(s, 5, 1);
+        IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
+        launch_wavespeed(s->g, s->storage, s->st[s->cur], (float)s->gamma, s->wave, s->stream);
+        s->wave_valid = (s->cur == 0);
+    }
+    WaveResult h;
+    IGR_CUDA_OK(cudaMemcpyAsync(&h, s->wave, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    int rc = finish(s, "igr_max_wavespeed");
+    if (rc != IGR_OK) return rc;
+    float v;
+    memcpy(&v, &h.max_bits, 4);
+    *out = (double)v;
+    if (h.nonfinite || !(v > 0.0f) || !std::isfinite(v))
+        return s->fail(IGR_ERR_NONFINITE, "igr_max_wavespeed: non-finite state (NaN/Inf, or negative pressure/density)");
+    return IGR_OK;
+}
+
+int igr_kernel_launches(igr_solver *s, long long *out)
+{
+    if (!s || !out) return IGR_ERR_ARG;
+    *out = s->launches;
+    return IGR_OK;
+}
+
+int igr_profile(igr_solver *s, int enable)
+{
+    if (!s) return IGR_ERR_ARG;
+    IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
+    s->ev.clear(); s->ev_row.clear();
+    s->profile = enable != 0;
+    return IGR_OK;
+}
+
+int igr_profile_read(igr_solver *s, double ms[6], long long count[6])
+{
+    if (!s || !ms || !count) return IGR_ERR_ARG;
+    IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+    for (int r = 0; r < 6; ++r) { ms[r] = 0.0; count[r] = 0; }
+    for (size_t i = 0; i < s->ev_row.size(); ++i) {
+        float t = 0.f;
+        IGR_CUDA_OK(cudaEventElapsedTime(&t, s->ev[2 * i], s->ev[2 * i + 1]));
+        ms[s->ev_row[i]] += t; count[s->ev_row[i]] += 1;
+    }
+    return IGR_OK;
+}
+
+}  // extern "C"

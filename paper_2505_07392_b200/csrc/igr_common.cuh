@@ -1,0 +1,70 @@
+// igr_common.cuh -- shared device/host definitions of libigr (B200, sm_100a).
+//
+// Data layout in HBM: every field is a padded SoA array
+//   f[(k + NG) * PY + (j + NG)][i + GX],   pitch PX elements, x fastest,
+// NG = 3 ghost layers in y and z, GX = 32 bytes of ghost/padding in x (8 fp32 / 16 half elements,
+// of which the 3 next to the interior are the ghost cells), PX = round_up(nx + 2 GX, 32 bytes).
+// Interior rows therefore start 32-byte aligned (sector aligned) and all TMA strides are
+// multiples of 16 bytes.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#define IGR_NG 3
+
+struct Grid {
+    int nx, ny, nz;        // interior cells
+    int gx;                // x ghost/padding elements (>= 3)
+    int px, py, pz;        // padded extents (elements)
+    long long sy, sz;      // strides in elements: sy = px, sz = px * py
+    long long np;          // px * py * pz
+    int bc[6];             // IGR_BC_* per face
+    __host__ __device__ long long idx(int i, int j, int k) const {   // interior-relative indices
+        return (long long)(i + gx) + sy * (long long)(j + IGR_NG) + sz * (long long)(k + IGR_NG);
+    }
+};
+
+// index map of the boundary conditions (reading A8): periodic -> wrap, otherwise clamp
+__host__ __device__ inline int map_index(int i, int n, int bc_lo)
+{
+    if (i >= 0 && i < n) return i;
+    if (bc_lo == 0) { int m = i % n; return m < 0 ? m + n : m; }
+    return i < 0 ? 0 : n - 1;
+}
+
+// ---- storage <-> fp32 (FP16 storage, FP32 compute)
+__device__ __forceinline__ float ldf(const float *p) { return *p; }
+__device__ __forceinline__ float ldf(const __half *p) { return __half2float(*p); }
+__device__ __forceinline__ float ldf(const __nv_bfloat16 *p) { return __bfloat162float(*p); }
+__device__ __forceinline__ void stf(float *p, float v) { *p = v; }
+__device__ __forceinline__ void stf(__half *p, float v) { *p = __float2half_rn(v); }
+__device__ __forceinline__ void stf(__nv_bfloat16 *p, float v) { *p = __float2bfloat16_rn(v); }
+
+struct StagePtrs {            // device pointers of one state buffer (5 padded fields)
+    void *f[5];
+};
+
+// inflow description of one face, device resident (weights precomputed on the host in fp64)
+struct InflowFace {
+    const float *weight;      // [n1][n0] blend weight w in [0,1] per transverse cell (NULL: none)
+    const float *fixed;       // [n1][n0][5] fixed conserved state of the winning patch
+    int n0, n1;               // transverse extents
+};
+
+struct BcDesc {
+    InflowFace inflow[6];
+};
+
+// ordered-int encoding of non-negative floats for atomicMax
+struct WaveResult {
+    unsigned int max_bits;    // float bits of the maximum wave speed (non-negative)
+    unsigned int nonfinite;   // != 0 if any cell produced a non-finite value
+};
+
+#define IGR_CUDA_OK(call)                                                                          \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) return s->fail(IGR_ERR_CUDA, #call, e_);                            \
+    } while (0)

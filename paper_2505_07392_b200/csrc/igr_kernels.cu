@@ -1,0 +1,490 @@
+// igr_kernels.cu -- boundary/halo, source, simple Jacobi sweep, simple RHS, RK update and the
+// wave-speed reduction of libigr (sm_100a).  Citations are PAPER.md lines; readings are DESIGN.md's.
+// The tiled/TMA RHS kernel and the temporally blocked Jacobi kernel live in their own files.
+#include "igr_kernels.h"
+
+#define IGR_STORE_F32 0
+#define IGR_STORE_F16 1
+#define IGR_STORE_BF16 2
+
+#define DISPATCH_STORAGE(storage, ...)                                                             \
+    do {                                                                                           \
+        if ((storage) == IGR_STORE_F32) { typedef float T; __VA_ARGS__; }                          \
+        else if ((storage) == IGR_STORE_F16) { typedef __half T; __VA_ARGS__; }                    \
+        else { typedef __nv_bfloat16 T; __VA_ARGS__; }                                             \
+    } while (0)
+
+static inline unsigned int blocks_for(long long n, int threads, long long cap = 1 << 20)
+{
+    long long b = (n + threads - 1) / threads;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (unsigned int)b;
+}
+
+// ------------------------------------------------------------------------------ pack / unpack
+template <typename T>
+__global__ void k_unpack(Grid g, const float *__restrict__ user, T *__restrict__ field, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx);
+        long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        stf(field + g.idx(i, j, k0 + k), user[t]);
+    }
+}
+
+template <typename T>
+__global__ void k_pack(Grid g, const T *__restrict__ field, float *__restrict__ user, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx);
+        long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        user[t] = ldf(field + g.idx(i, j, k0 + k));
+    }
+}
+
+template <typename T>
+__global__ void k_pack_padded(Grid g, const T *__restrict__ field, float *__restrict__ user, int k0, int nk)
+{
+    const int wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG;
+    long long n = (long long)nk * wy * wx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % wx);
+        long long r = t / wx;
+        int j = (int)(r % wy), k = (int)(r / wy);
+        user[t] = ldf(field + g.idx(i - IGR_NG, j - IGR_NG, k0 + k - IGR_NG));
+    }
+}
+
+void launch_unpack_field(const Grid &g, int storage, const float *user, void *field, int k0, int nk,
+                         cudaStream_t st)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    DISPATCH_STORAGE(storage, k_unpack<T><<<blocks_for(n, 256), 256, 0, st>>>(g, user, (T *)field, k0, nk));
+}
+
+void launch_pack_field(const Grid &g, int storage, const void *field, float *user, int k0, int nk,
+                       cudaStream_t st)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    DISPATCH_STORAGE(storage, k_pack<T><<<blocks_for(n, 256), 256, 0, st>>>(g, (const T *)field, user, k0, nk));
+}
+
+void launch_unpack_f32(const Grid &g, const float *user, float *field, int k0, int nk, cudaStream_t st)
+{
+    launch_unpack_field(g, IGR_STORE_F32, user, field, k0, nk, st);
+}
+
+void launch_pack_f32(const Grid &g, const float *field, float *user, int k0, int nk, cudaStream_t st)
+{
+    launch_pack_field(g, IGR_STORE_F32, field, user, k0, nk, st);
+}
+
+void launch_pack_padded(const Grid &g, int storage, const void *field, float *user, int k0, int nk,
+                        cudaStream_t st)
+{
+    long long n = (long long)nk * (g.ny + 2 * IGR_NG) * (g.nx + 2 * IGR_NG);
+    DISPATCH_STORAGE(storage,
+                     k_pack_padded<T><<<blocks_for(n, 256), 256, 0, st>>>(g, (const T *)field, user, k0, nk));
+}
+
+// ------------------------------------------------------------------------------ a1: halo / BC
+// The paper gives no boundary conditions; BASELINE.json names periodic, extrapolation outflow and
+// fixed-state inflow patches.  Reading A8: every ghost cell is a copy of the interior cell given by
+// the per-axis index map (wrap / clamp), blended towards the fixed patch state on inflow faces.
+// All ghosts read interior cells only, so one launch covers the three slabs (no ordering).
+struct GhostCell { int i, j, k; bool valid; };
+
+__device__ __forceinline__ GhostCell decode_ghost(const Grid &g, long long t)
+{
+    const int wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG;
+    const long long nZ = 2LL * IGR_NG * wy * wx;                 // full padded planes below/above
+    const long long nY = (long long)g.nz * 2 * IGR_NG * wx;      // rows in front/behind, interior k
+    const long long nX = (long long)g.nz * g.ny * 2 * IGR_NG;    // columns left/right, interior j, k
+    GhostCell c;
+    c.valid = true;
+    if (t < nZ) {
+        int i = (int)(t % wx); long long r = t / wx;
+        int j = (int)(r % wy), kk = (int)(r / wy);
+        c.i = i - IGR_NG; c.j = j - IGR_NG; c.k = kk < IGR_NG ? kk - IGR_NG : g.nz + (kk - IGR_NG);
+    } else if (t < nZ + nY) {
+        t -= nZ;
+        int i = (int)(t % wx); long long r = t / wx;
+        int jj = (int)(r % (2 * IGR_NG)); c.k = (int)(r / (2 * IGR_NG));
+        c.i = i - IGR_NG; c.j = jj < IGR_NG ? jj - IGR_NG : g.ny + (jj - IGR_NG);
+    } else if (t < nZ + nY + nX) {
+        t -= nZ + nY;
+        int ii = (int)(t % (2 * IGR_NG)); long long r = t / (2 * IGR_NG);
+        c.j = (int)(r % g.ny); c.k = (int)(r / g.ny);
+        c.i = ii < IGR_NG ? ii - IGR_NG : g.nx + (ii - IGR_NG);
+    } else {
+        c.valid = false; c.i = c.j = c.k = 0;
+    }
+    return c;
+}
+
+__host__ __device__ inline long long ghost_count(const Grid &g)
+{
+    const long long wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG;
+    return 2LL * IGR_NG * wy * wx + (long long)g.nz * 2 * IGR_NG * wx + (long long)g.nz * g.ny * 2 * IGR_NG;
+}
+
+template <typename T>
+__global__ void k_halo_q(Grid g, StagePtrs q, BcDesc bc)
+{
+    const long long n = ghost_count(g);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        GhostCell c = decode_ghost(g, t);
+        const long long dst = g.idx(c.i, c.j, c.k);
+        const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
+                                    map_index(c.k, g.nz, g.bc[4]));
+        // inflow: first out-of-range axis (x, y, z order) whose face is an inflow face
+        float w = 0.f;
+        const float *fixed = nullptr;
+        const int idx[3] = { c.i, c.j, c.k }, nn[3] = { g.nx, g.ny, g.nz };
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            int face = idx[a] < 0 ? 2 * a : (idx[a] >= nn[a] ? 2 * a + 1 : -1);
+            if (face < 0 || fixed != nullptr) continue;
+            const InflowFace &f = bc.inflow[face];
+            if (f.weight == nullptr) continue;
+            int t0 = (a == 0) ? idx[1] : idx[0];
+            int t1 = (a == 2) ? idx[1] : idx[2];
+            if (t0 < 0 || t0 >= f.n0 || t1 < 0 || t1 >= f.n1) continue;   // edge/corner ghosts: never read
+            float ww = f.weight[(long long)t1 * f.n0 + t0];
+            if (ww > 0.f) { w = ww; fixed = f.fixed + ((long long)t1 * f.n0 + t0) * 5; }
+        }
+#pragma unroll
+        for (int cmp = 0; cmp < 5; ++cmp) {
+            T *fld = (T *)q.f[cmp];
+            float v = ldf(fld + src);
+            if (fixed != nullptr) v = (w >= 1.f) ? fixed[cmp] : v + w * (fixed[cmp] - v);
+            stf(fld + dst, v);
+        }
+    }
+}
+
+template <typename T>
+__global__ void k_halo_sigma(Grid g, T *__restrict__ sig)
+{
+    // Sigma ghosts: wrap on periodic faces, clamp on every other face (homogeneous Neumann, A8)
+    const long long n = ghost_count(g);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        GhostCell c = decode_ghost(g, t);
+        const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
+                                    map_index(c.k, g.nz, g.bc[4]));
+        sig[g.idx(c.i, c.j, c.k)] = sig[src];
+    }
+}
+
+void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cudaStream_t st)
+{
+    long long n = ghost_count(g);
+    DISPATCH_STORAGE(storage, k_halo_q<T><<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, q, bc));
+}
+
+void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
+{
+    long long n = ghost_count(g);
+    DISPATCH_STORAGE(storage, k_halo_sigma<T><<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, (T *)sig));
+}
+
+// ------------------------------------------------------------------------------ a2: source
+// b = alpha ( tr((grad u)^2) + (tr grad u)^2 )  -- the side of eq. (9) that carries alpha (L127,
+// footnote L252) with second-order central differences of the cell-centred velocity u = m/rho
+// (L132; Alg. 1).  G_ab = d u_a / d x_b.
+template <typename T>
+__global__ void k_source(Grid g, StagePtrs q, float *__restrict__ b, float alpha, float inv2dx)
+{
+    const T *rho = (const T *)q.f[0];
+    const T *m[3] = { (const T *)q.f[1], (const T *)q.f[2], (const T *)q.f[3] };
+    const long long st[3] = { 1, g.sy, g.sz };
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        float G[3][3];
+#pragma unroll
+        for (int bb = 0; bb < 3; ++bb) {
+            const long long ip = id + st[bb], im = id - st[bb];
+            const float rp = 1.0f / ldf(rho + ip), rm = 1.0f / ldf(rho + im);
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                G[a][bb] = (ldf(m[a] + ip) * rp - ldf(m[a] + im) * rm) * inv2dx;
+        }
+        const float tr = G[0][0] + G[1][1] + G[2][2];
+        const float trsq = G[0][0] * G[0][0] + G[1][1] * G[1][1] + G[2][2] * G[2][2] +
+                           2.0f * (G[0][1] * G[1][0] + G[0][2] * G[2][0] + G[1][2] * G[2][1]);
+        b[id] = alpha * (trsq + tr * tr);
+    }
+}
+
+void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
+                   cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    DISPATCH_STORAGE(storage, k_source<T><<<blocks_for(n, 256), 256, 0, st>>>(g, q, b, alpha, inv2dx));
+}
+
+// ------------------------------------------------------------------------------ a3: Jacobi sweep
+// Sigma/rho - alpha div(grad(Sigma)/rho) = b  (eq. 9, reading A1) on the 6-point stencil (L138),
+// face density = arithmetic mean (reading A2):
+//   Sigma_i <- ( b_i + k2 sum_n w_in Sigma_n ) / ( 1/rho_i + k2 sum_n w_in ),  w_in = 2/(rho_i + rho_n),
+// k2 = alpha/dx^2.  Ghost values of the iterate follow the BC index map at every sweep (wrap /
+// clamp), so the neighbour index is mapped instead of refreshing ghosts between sweeps; rho ghosts
+// come from the filled q ghosts.
+template <typename T>
+__global__ void k_jacobi_sweep(Grid g, const T *__restrict__ rho, const float *__restrict__ b,
+                               const T *__restrict__ sin, T *__restrict__ sout, float k2)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        const float rc = ldf(rho + id);
+        float num = 0.f, den = 0.f;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int sgn = -1; sgn <= 1; sgn += 2) {
+                int ii = i + (a == 0 ? sgn : 0), jj = j + (a == 1 ? sgn : 0), kk = k + (a == 2 ? sgn : 0);
+                const float w = 2.0f / (rc + ldf(rho + g.idx(ii, jj, kk)));
+                const long long ns = g.idx(map_index(ii, g.nx, g.bc[0]), map_index(jj, g.ny, g.bc[2]),
+                                           map_index(kk, g.nz, g.bc[4]));
+                num += w * ldf(sin + ns);
+                den += w;
+            }
+        }
+        stf(sout + id, (b[id] + k2 * num) / (1.0f / rc + k2 * den));
+    }
+}
+
+void launch_jacobi_sweep(const Grid &g, int storage, const void *rho, const float *b,
+                         const void *sig_in, void *sig_out, float k2, cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    DISPATCH_STORAGE(storage, k_jacobi_sweep<T><<<blocks_for(n, 256), 256, 0, st>>>(
+                                  g, (const T *)rho, b, (const T *)sig_in, (T *)sig_out, k2));
+}
+
+// ------------------------------------------------------------------------------ a4: RHS, simple form
+// Reference-quality kernel (one thread per cell, both faces of each direction recomputed, global
+// loads through L1/L2).  It defines the arithmetic the tiled kernel must reproduce:
+//   reconstruction of (rho, m, E, Sigma) at the face from cells -2..3 (L132, L164, Alg. 1,
+//   L205), primitives from the reconstructed conservative values (L187-L198), flux with p + Sigma
+//   (eqs. 6-8), Lax-Friedrichs with lambda = max(|u_d| + c) of the two adjacent
+//   cell-centred states (L132, L207-L210; reading A5), r = -sum_d (F^_{i+1/2} - F^_{i-1/2})/dx.
+template <int ORDER>
+__device__ __forceinline__ void reconstruct(const float f[6], float &fl, float &fr)
+{
+    if (ORDER == 5) {
+        fl = (2.f / 60.f) * f[0] + (-13.f / 60.f) * f[1] + (47.f / 60.f) * f[2] + (27.f / 60.f) * f[3] + (-3.f / 60.f) * f[4];
+        fr = (-3.f / 60.f) * f[1] + (27.f / 60.f) * f[2] + (47.f / 60.f) * f[3] + (-13.f / 60.f) * f[4] + (2.f / 60.f) * f[5];
+    } else {
+        fl = (-1.f / 6.f) * f[1] + (5.f / 6.f) * f[2] + (2.f / 6.f) * f[3];
+        fr = (2.f / 6.f) * f[2] + (5.f / 6.f) * f[3] + (-1.f / 6.f) * f[4];
+    }
+}
+
+__device__ __forceinline__ void side_flux(int d, float gm1, const float U[5], float sg, float F[5])
+{
+    const float ir = 1.0f / U[0];
+    const float ud = U[1 + d] * ir;
+    const float p = gm1 * (U[4] - 0.5f * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * ir);
+    F[0] = U[1 + d];
+    F[1] = U[1] * ud; F[2] = U[2] * ud; F[3] = U[3] * ud;
+    F[1 + d] += p + sg;
+    F[4] = (U[4] + p + sg) * ud;
+}
+
+template <typename T>
+__device__ __forceinline__ float cell_wavespeed(int d, float gamma, const StagePtrs &q, long long id)
+{
+    const float rho = ldf((const T *)q.f[0] + id), ir = 1.0f / rho;
+    const float mx = ldf((const T *)q.f[1] + id), my = ldf((const T *)q.f[2] + id), mz = ldf((const T *)q.f[3] + id);
+    const float p = (gamma - 1.0f) * (ldf((const T *)q.f[4] + id) - 0.5f * (mx * mx + my * my + mz * mz) * ir);
+    const float md = d == 0 ? mx : (d == 1 ? my : mz);
+    return fabsf(md * ir) + sqrtf(gamma * p * ir);
+}
+
+// numerical flux at the face between cell `id` and `id + stride` along d
+template <typename T, int ORDER>
+__device__ __forceinline__ void face_flux(int d, const StagePtrs &q, const T *sig, long long id,
+                                          long long stride, float gamma, float F[5])
+{
+    float UL[5], UR[5], f[6], sl, sr;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+#pragma unroll
+        for (int t = 0; t < 6; ++t) f[t] = ldf((const T *)q.f[c] + id + (t - 2) * stride);
+        reconstruct<ORDER>(f, UL[c], UR[c]);
+    }
+#pragma unroll
+    for (int t = 0; t < 6; ++t) f[t] = ldf(sig + id + (t - 2) * stride);
+    reconstruct<ORDER>(f, sl, sr);
+    const float lam = fmaxf(cell_wavespeed<T>(d, gamma, q, id), cell_wavespeed<T>(d, gamma, q, id + stride));
+    float FL[5], FR[5];
+    side_flux(d, gamma - 1.0f, UL, sl, FL);
+    side_flux(d, gamma - 1.0f, UR, sr, FR);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) F[c] = 0.5f * (FL[c] + FR[c]) - 0.5f * lam * (UR[c] - UL[c]);
+}
+
+template <typename T, int ORDER>
+__global__ void k_rhs_simple(Grid g, StagePtrs q, const T *__restrict__ sig, float *r0, float *r1,
+                             float *r2, float *r3, float *r4, float gamma, float inv_dx)
+{
+    float *rr[5] = { r0, r1, r2, r3, r4 };
+    const long long st[3] = { 1, g.sy, g.sz };
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        float acc[5] = { 0.f, 0.f, 0.f, 0.f, 0.f };
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            float Fp[5], Fm[5];
+            face_flux<T, ORDER>(d, q, sig, id, st[d], gamma, Fp);
+            face_flux<T, ORDER>(d, q, sig, id - st[d], st[d], gamma, Fm);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) acc[c] -= (Fp[c] - Fm[c]) * inv_dx;
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) rr[c][id] = acc[c];
+    }
+}
+
+void launch_rhs_simple(const Grid &g, int storage, StagePtrs q, const void *sig, float *const r[5],
+                       RhsParams p, cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    unsigned int nb = blocks_for(n, 128);
+    DISPATCH_STORAGE(storage, {
+        if (p.order == 5)
+            k_rhs_simple<T, 5><<<nb, 128, 0, st>>>(g, q, (const T *)sig, r[0], r[1], r[2], r[3], r[4], p.gamma, p.inv_dx);
+        else
+            k_rhs_simple<T, 3><<<nb, 128, 0, st>>>(g, q, (const T *)sig, r[0], r[1], r[2], r[3], r[4], p.gamma, p.inv_dx);
+    });
+}
+
+// ------------------------------------------------------------------------------ a5/a6: update, wave speed
+// SSP-RK3 of Gottlieb & Shu (L138, ref. 17 L389): every stage is a convex combination
+//   q_out = a q_n + beta (q_s + dt r),  a + beta = 1,  beta = 1, 1/4, 2/3,
+// evaluated as q_n + beta ((q_s - q_n) + dt r) so that r = 0, q_s = q_n returns q_n bitwise (A18).
+// With `wave` the kernel also reduces max(|u_d|) + c of the NEW state (warp shuffle, then one
+// atomicMax per block on the float bits, valid for non-negative floats) and flags non-finite cells.
+__device__ __forceinline__ void block_reduce_wave(float v, bool bad, WaveResult *wave)
+{
+    __shared__ float s_max[32];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) s_bad = 0;
+    __syncthreads();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    bad = __any_sync(0xffffffffu, bad);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { s_max[wid] = v; if (bad) atomicOr(&s_bad, 1); }
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        v = lane < nw ? s_max[lane] : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if (lane == 0) {
+            atomicMax(&wave->max_bits, __float_as_uint(v));
+            if (s_bad) atomicOr(&wave->nonfinite, 1u);
+        }
+    }
+}
+
+__device__ __forceinline__ float wavespeed_of(float rho, float mx, float my, float mz, float E,
+                                              float gamma, bool &bad)
+{
+    const float ir = 1.0f / rho;
+    const float p = (gamma - 1.0f) * (E - 0.5f * (mx * mx + my * my + mz * mz) * ir);
+    const float v = fmaxf(fabsf(mx), fmaxf(fabsf(my), fabsf(mz))) * fabsf(ir) + sqrtf(gamma * p * ir);
+    // non-finite (NaN/Inf, or sqrt of a negative) is reported, never repaired (reading A10)
+    if (!(v <= 3.0e38f)) { bad = true; return 0.f; }
+    return v;
+}
+
+template <typename T, bool WAVE>
+__global__ void k_rk_update(Grid g, StagePtrs qn, StagePtrs qs, StagePtrs qo, const float *r0,
+                            const float *r1, const float *r2, const float *r3, const float *r4,
+                            float beta, float dt, float gamma, WaveResult *wave)
+{
+    const float *rr[5] = { r0, r1, r2, r3, r4 };
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    float vmax = 0.f;
+    bool bad = false;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        float o[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            const float a = ldf((const T *)qn.f[c] + id), s = ldf((const T *)qs.f[c] + id);
+            o[c] = a + beta * ((s - a) + dt * rr[c][id]);
+            stf((T *)qo.f[c] + id, o[c]);
+            if (WAVE) o[c] = ldf((const T *)qo.f[c] + id);      // wave speed of the STORED state
+        }
+        if (WAVE) vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], gamma, bad));
+    }
+    if (WAVE) block_reduce_wave(vmax, bad, wave);
+}
+
+void launch_rk_update(const Grid &g, int storage, StagePtrs qn, StagePtrs qs, StagePtrs qout,
+                      float *const r[5], float beta, float dt, float gamma, WaveResult *wave,
+                      cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    unsigned int nb = blocks_for(n, 256, 148 * 8);
+    DISPATCH_STORAGE(storage, {
+        if (wave)
+            k_rk_update<T, true><<<nb, 256, 0, st>>>(g, qn, qs, qout, r[0], r[1], r[2], r[3], r[4], beta, dt, gamma, wave);
+        else
+            k_rk_update<T, false><<<nb, 256, 0, st>>>(g, qn, qs, qout, r[0], r[1], r[2], r[3], r[4], beta, dt, gamma, wave);
+    });
+}
+
+template <typename T>
+__global__ void k_wavespeed(Grid g, StagePtrs q, float gamma, WaveResult *wave)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    float vmax = 0.f;
+    bool bad = false;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        vmax = fmaxf(vmax, wavespeed_of(ldf((const T *)q.f[0] + id), ldf((const T *)q.f[1] + id),
+                                        ldf((const T *)q.f[2] + id), ldf((const T *)q.f[3] + id),
+                                        ldf((const T *)q.f[4] + id), gamma, bad));
+    }
+    block_reduce_wave(vmax, bad, wave);
+}
+
+void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, WaveResult *wave,
+                      cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    DISPATCH_STORAGE(storage, k_wavespeed<T><<<blocks_for(n, 256, 148 * 8), 256, 0, st>>>(g, q, gamma, wave));
+}

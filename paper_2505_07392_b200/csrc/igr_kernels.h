@@ -1,0 +1,47 @@
+// igr_kernels.h -- host-side launchers of the CUDA kernels of libigr (one per row of the hot path,
+// SURVEY.md 8(a)).  `storage` is IGR_STORE_F32 / F16 / BF16 (igr.h); q and Sigma use that element
+// type, b and r are always fp32.
+#pragma once
+#include "igr_common.cuh"
+
+struct RhsParams {
+    float gamma, inv_dx;
+    int order;
+};
+
+// interior <-> padded copies.  `user` is a DEVICE fp32 array holding planes [k0, k0+nk) of one
+// field, layout [nk][ny][nx].
+void launch_unpack_field(const Grid &g, int storage, const float *user, void *field, int k0, int nk,
+                         cudaStream_t st);
+void launch_pack_field(const Grid &g, int storage, const void *field, float *user, int k0, int nk,
+                       cudaStream_t st);
+void launch_unpack_f32(const Grid &g, const float *user, float *field, int k0, int nk, cudaStream_t st);
+void launch_pack_f32(const Grid &g, const float *field, float *user, int k0, int nk, cudaStream_t st);
+// padded copy with 3 ghost layers: out [nz+6][ny+6][nx+6] planes [k0,k0+nk) of the padded z range
+void launch_pack_padded(const Grid &g, int storage, const void *field, float *user, int k0, int nk,
+                        cudaStream_t st);
+
+// a1: ghosts of q (5 fields) / of Sigma
+void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cudaStream_t st);
+void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st);
+
+// a2: b = alpha (tr((grad u)^2) + (tr grad u)^2)
+void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
+                   cudaStream_t st);
+
+// a3 (simple form): one Jacobi sweep, neighbours of Sigma through the BC index map
+void launch_jacobi_sweep(const Grid &g, int storage, const void *rho, const float *b,
+                         const void *sig_in, void *sig_out, float k2, cudaStream_t st);
+
+// a4 (simple form): r = -div F^
+void launch_rhs_simple(const Grid &g, int storage, StagePtrs q, const void *sig, float *const r[5],
+                       RhsParams p, cudaStream_t st);
+
+// a5: q_out = q_n + beta ((q_s - q_n) + dt r); if `wave` != NULL also reduces the wave speed of q_out
+void launch_rk_update(const Grid &g, int storage, StagePtrs qn, StagePtrs qs, StagePtrs qout,
+                      float *const r[5], float beta, float dt, float gamma, WaveResult *wave,
+                      cudaStream_t st);
+
+// a6: wave = max_cells(max_d |u_d| + c), non-finite flag
+void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, WaveResult *wave,
+                      cudaStream_t st);

@@ -1,0 +1,241 @@
+"""Thin Python binding of libigr.so (include/igr.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the library.  PyTorch is used for device
+memory (the solver's workspace is a torch tensor) and for the stream.  There is no CPU fallback:
+loading fails loudly if the library has not been built, and igr_create fails without a GPU.
+Names follow include/igr.h (igr_create -> Solver(...), igr_step -> Solver.step, ...).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libigr.so")
+
+OK, ERR_ARG, ERR_BC, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
+BC_PERIODIC, BC_EXTRAP, BC_INFLOW = 0, 1, 2
+STORE_F32, STORE_F16, STORE_BF16 = 0, 1, 2
+_STATUS = {0: "IGR_OK", -1: "IGR_ERR_ARG", -2: "IGR_ERR_BC", -3: "IGR_ERR_ALLOC", -4: "IGR_ERR_CUDA",
+           -5: "IGR_ERR_NONFINITE"}
+
+EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", "igr_set_state",
+           "igr_get_state", "igr_set_sigma", "igr_get_sigma", "igr_max_wavespeed", "igr_step",
+           "igr_sync", "igr_last_error", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs",
+           "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
+           "igr_kernel_launches", "igr_profile", "igr_profile_read"]
+
+
+class IgrError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__("%s (%d) %s" % (_STATUS.get(code, "?"), code, msg))
+
+
+class Patch(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("c0", "c1", "radius", "edge", "rho", "u", "v", "w", "p")]
+
+
+class BC(C.Structure):
+    _fields_ = [("face", C.c_int32 * 6), ("n_patches", C.c_int32 * 6),
+                ("patches", C.POINTER(Patch) * 6)]
+
+
+class Options(C.Structure):
+    _fields_ = [("storage", C.c_int32), ("fused", C.c_int32), ("stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libigr.so; raises if it has not been built (python -m paper_2505_07392_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libigr.so is missing: build it with `python -m paper_2505_07392_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, fp = C.c_void_p, C.c_void_p          # float pointers are passed as raw addresses
+        L.igr_workspace_bytes.argtypes = [C.c_int] * 3 + [C.POINTER(Options)]
+        L.igr_workspace_bytes.restype = C.c_size_t
+        L.igr_create.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int] * 2 + [C.POINTER(BC), C.POINTER(vp)]
+        L.igr_create_ex.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int] * 2 + \
+            [C.POINTER(BC), C.POINTER(Options), C.POINTER(vp)]
+        L.igr_destroy.argtypes = [vp]
+        L.igr_destroy.restype = None
+        for n in ("igr_set_state", "igr_get_state", "igr_set_sigma", "igr_get_sigma", "igr_get_source",
+                  "igr_set_source", "igr_get_rhs"):
+            getattr(L, n).argtypes = [vp, fp]
+        L.igr_get_padded.argtypes = [vp, C.c_int, fp]
+        L.igr_max_wavespeed.argtypes = [vp, C.POINTER(C.c_double)]
+        L.igr_step.argtypes = [vp, C.c_double]
+        L.igr_rk_update.argtypes = [vp, C.c_int, C.c_double]
+        for n in ("igr_sync", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs"):
+            getattr(L, n).argtypes = [vp]
+        L.igr_kernel_launches.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.igr_profile.argtypes = [vp, C.c_int]
+        L.igr_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.igr_last_error.argtypes = [vp]
+        L.igr_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def make_bc(faces, patches=None):
+    """faces: 6 codes (x-,x+,y-,y+,z-,z+); patches: {face: [(c0,c1,radius,edge,rho,u,v,w,p), ...]}"""
+    bc, keep = BC(), []
+    for f in range(6):
+        bc.face[f] = int(faces[f])
+        plist = (patches or {}).get(f, [])
+        bc.n_patches[f] = len(plist)
+        if plist:
+            arr = (Patch * len(plist))(*[Patch(*map(float, p)) for p in plist])
+            keep.append(arr)
+            bc.patches[f] = C.cast(arr, C.POINTER(Patch))
+    return bc, keep
+
+
+def _addr(a, shape, writable=False):
+    """Raw address of a contiguous fp32 torch tensor (cpu or cuda) or numpy array of `shape`."""
+    if isinstance(a, torch.Tensor):
+        assert a.dtype == torch.float32 and a.is_contiguous() and tuple(a.shape) == tuple(shape), \
+            (a.dtype, a.shape, shape)
+        return a.data_ptr()
+    assert isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous \
+        and a.shape == tuple(shape), (type(a), getattr(a, "shape", None), shape)
+    if writable:
+        assert a.flags.writeable
+    return a.ctypes.data
+
+
+class Solver:
+    """igr_create_ex / igr_destroy and the calls of include/igr.h on one solver object."""
+
+    def __init__(self, nx, ny, nz, dx, gamma, alpha, order=5, n_jacobi=5, faces=(0,) * 6, patches=None,
+                 storage=STORE_F32, fused=0, device="cuda:0", own_workspace=True):
+        L = lib()
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.shape = (nz, ny, nx)
+        self.device = torch.device(device)
+        self._h = None
+        opt = Options()
+        opt.storage, opt.fused = storage, fused
+        if not torch.cuda.is_available():
+            raise IgrError(ERR_CUDA, "no CUDA device: libigr has no CPU fallback")
+        torch.cuda.set_device(self.device)
+        self.stream = torch.cuda.current_stream(self.device)
+        opt.stream = self.stream.cuda_stream
+        if own_workspace:
+            nbytes = L.igr_workspace_bytes(nx, ny, nz, C.byref(opt))
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            opt.workspace, opt.workspace_bytes = base, nbytes
+        bc, self._keep = make_bc(faces, patches)
+        h = C.c_void_p()
+        rc = L.igr_create_ex(nx, ny, nz, dx, gamma, alpha, order, n_jacobi, C.byref(bc), C.byref(opt),
+                             C.byref(h))
+        if rc != OK:
+            raise IgrError(rc, "igr_create_ex")
+        self._h = h
+
+    @classmethod
+    def for_workload(cls, w, **kw):
+        return cls(w.nx, w.ny, w.nz, w.dx, w.gamma, w.alpha, order=w.order, n_jacobi=w.n_jacobi,
+                   faces=w.faces, patches=w.patches, **kw)
+
+    def close(self):
+        if self._h:
+            lib().igr_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != OK:
+            raise IgrError(rc, lib().igr_last_error(self._h).decode())
+
+    # ---- igr.h calls
+    def set_state(self, q):
+        self._check(lib().igr_set_state(self._h, _addr(q, (5,) + self.shape)))
+
+    def get_state(self, out=None):
+        out = np.empty((5,) + self.shape, np.float32) if out is None else out
+        self._check(lib().igr_get_state(self._h, _addr(out, (5,) + self.shape, True)))
+        return out
+
+    def set_sigma(self, f):
+        self._check(lib().igr_set_sigma(self._h, _addr(f, self.shape)))
+
+    def _scalar_out(self, fn, out):
+        out = np.empty(self.shape, np.float32) if out is None else out
+        self._check(fn(self._h, _addr(out, self.shape, True)))
+        return out
+
+    def get_sigma(self, out=None):
+        return self._scalar_out(lib().igr_get_sigma, out)
+
+    def get_source(self, out=None):
+        return self._scalar_out(lib().igr_get_source, out)
+
+    def set_source(self, f):
+        self._check(lib().igr_set_source(self._h, _addr(f, self.shape)))
+
+    def get_rhs(self, out=None):
+        out = np.empty((5,) + self.shape, np.float32) if out is None else out
+        self._check(lib().igr_get_rhs(self._h, _addr(out, (5,) + self.shape, True)))
+        return out
+
+    def get_padded(self, c, out=None):
+        shp = (self.nz + 6, self.ny + 6, self.nx + 6)
+        out = np.empty(shp, np.float32) if out is None else out
+        self._check(lib().igr_get_padded(self._h, c, _addr(out, shp, True)))
+        return out
+
+    def max_wavespeed(self):
+        v = C.c_double()
+        self._check(lib().igr_max_wavespeed(self._h, C.byref(v)))
+        return v.value
+
+    def step(self, dt):
+        self._check(lib().igr_step(self._h, float(dt)))
+
+    def sync(self):
+        self._check(lib().igr_sync(self._h))
+
+    def halo_bc(self):
+        self._check(lib().igr_halo_bc(self._h))
+
+    def sigma_source(self):
+        self._check(lib().igr_sigma_source(self._h))
+
+    def jacobi(self):
+        self._check(lib().igr_jacobi(self._h))
+
+    def rhs(self):
+        self._check(lib().igr_rhs(self._h))
+
+    def rk_update(self, stage, dt):
+        self._check(lib().igr_rk_update(self._h, int(stage), float(dt)))
+
+    ROWS = ("halo_bc", "sigma_source", "jacobi", "rhs", "rk_update", "max_wavespeed")
+
+    def kernel_launches(self):
+        v = C.c_longlong()
+        self._check(lib().igr_kernel_launches(self._h, C.byref(v)))
+        return v.value
+
+    def profile(self, enable):
+        self._check(lib().igr_profile(self._h, int(bool(enable))))
+
+    def profile_read(self):
+        """{row: (total_ms, calls)} of the rows timed since profile(True)."""
+        ms, cnt = (C.c_double * 6)(), (C.c_longlong * 6)()
+        self._check(lib().igr_profile_read(self._h, ms, cnt))
+        return {r: (ms[i], cnt[i]) for i, r in enumerate(self.ROWS)}

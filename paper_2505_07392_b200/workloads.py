@@ -64,17 +64,18 @@ def hash_noise(gi, gj, gk, gshape, comp, seed):
     return h.to(torch.float64) * (2.0 / 4294967296.0) - 1.0
 
 
-def _index_grids(w, device):
+def _index_grids(w, device, kz0=0, nk=None):
     i0, j0, k0 = w.origin
+    nk = w.nz if nk is None else nk
     gi = torch.arange(w.nx, dtype=torch.int64, device=device).view(1, 1, -1) + i0
     gj = torch.arange(w.ny, dtype=torch.int64, device=device).view(1, -1, 1) + j0
-    gk = torch.arange(w.nz, dtype=torch.int64, device=device).view(-1, 1, 1) + k0
+    gk = torch.arange(nk, dtype=torch.int64, device=device).view(-1, 1, 1) + (k0 + kz0)
     return gi, gj, gk
 
 
-def _conserved(w, rho, u, v, ww, p, out_dtype):
+def _conserved(w, rho, u, v, ww, p, out_dtype, nk):
     """(rho, u, p) -> (rho, rho u, E) with E = p/(gamma-1) + rho |u|^2 / 2 (eq. 4)."""
-    shape = (w.nz, w.ny, w.nx)
+    shape = (nk, w.ny, w.nx)
     rho, u, v, ww, p = (torch.broadcast_to(t, shape) for t in (rho, u, v, ww, p))
     q = torch.empty((5,) + shape, dtype=out_dtype, device=rho.device)
     q[0] = rho
@@ -85,10 +86,23 @@ def _conserved(w, rho, u, v, ww, p, out_dtype):
     return q
 
 
-def state(w, device="cpu", dtype=torch.float32):
-    """Initial conserved state of workload `w`, [5][nz][ny][nx], generated on `device`."""
+def state(w, device="cpu", dtype=torch.float32, slab=None):
+    """Initial conserved state of workload `w`, [5][nz][ny][nx], generated on `device` (in z-slabs
+    so that the fp64 temporaries of the large cases stay small)."""
+    if slab is None:
+        slab = max(1, min(w.nz, (1 << 24) // (w.nx * w.ny) or 1))
+    if slab >= w.nz:
+        return _state_slab(w, device, dtype, 0, w.nz)
+    q = torch.empty((5, w.nz, w.ny, w.nx), dtype=dtype, device=torch.device(device))
+    for k0 in range(0, w.nz, slab):
+        nk = min(slab, w.nz - k0)
+        q[:, k0:k0 + nk] = _state_slab(w, device, dtype, k0, nk)
+    return q
+
+
+def _state_slab(w, device, dtype, kz0, nk):
     dev = torch.device(device)
-    gi, gj, gk = _index_grids(w, dev)
+    gi, gj, gk = _index_grids(w, dev, kz0, nk)
     f64 = torch.float64
     one = torch.ones((), dtype=f64, device=dev)
     x = (gi.to(f64) + 0.5) * w.dx
@@ -98,7 +112,7 @@ def state(w, device="cpu", dtype=torch.float32):
     P = w.params
     if w.kind == "entropy_wave":
         rho = 1.0 + 0.2 * torch.sin(2.0 * math.pi * (x + y + z))
-        return _conserved(w, rho, one, one, one, one, dtype)
+        return _conserved(w, rho, one, one, one, one, dtype, nk)
     if w.kind == "sod":
         # the interface is smoothed over `smooth` cells (tanh half-width): the purely linear
         # scheme does not survive a grid-sharp start with alpha = 10 dx^2 (recipe)
@@ -111,13 +125,13 @@ def state(w, device="cpu", dtype=torch.float32):
         if P["noise"] > 0:
             rho = rho * (1.0 + P["noise"] * hash_noise(gi, gj, gk, gshape, 0, P["seed"]))
         zero = 0.0 * one
-        return _conserved(w, rho, zero, zero, zero, p, dtype)
+        return _conserved(w, rho, zero, zero, zero, p, dtype, nk)
     if w.kind == "taylor_green":
         p0 = 1.0 / (w.gamma * P["mach"] ** 2)
         u = torch.sin(x) * torch.cos(y) * torch.cos(z)
         v = -torch.cos(x) * torch.sin(y) * torch.cos(z)
         p = p0 + (torch.cos(2 * x) + torch.cos(2 * y)) * (torch.cos(2 * z) + 2.0) / 16.0
-        return _conserved(w, one, u, v, 0.0 * one, p, dtype)
+        return _conserved(w, one, u, v, 0.0 * one, p, dtype, nk)
     if w.kind == "jets":
         amp, seed = P["noise"], P["seed"]
         # ambient at rest + a smoothed jet column above every inflow patch: the linear scheme
@@ -140,10 +154,10 @@ def state(w, device="cpu", dtype=torch.float32):
         u = amp * hash_noise(gi, gj, gk, gshape, 1, seed)
         v = amp * hash_noise(gi, gj, gk, gshape, 2, seed)
         ww = amp * hash_noise(gi, gj, gk, gshape, 3, seed) + w_j * s
-        return _conserved(w, rho, u, v, ww, p, dtype)
+        return _conserved(w, rho, u, v, ww, p, dtype, nk)
     if w.kind == "uniform":
         return _conserved(w, P["rho"] * one, P["u"] * one, P["v"] * one, P["w"] * one,
-                          P["p"] * one, dtype)
+                          P["p"] * one, dtype, nk)
     raise ValueError(w.kind)
 
 

@@ -1,0 +1,151 @@
+"""GPU parity on the five configurations of BASELINE.json, whole steps through the C ABI against
+the fp64 oracle on the same seeded inputs, with the dt replay of reading A16.
+
+Tolerances (north_star): fp32 vs fp64 oracle, max-rel <= 1e-4 on smooth cases (configs 1, 3),
+L1-rel <= 1e-3 on shocked cases (configs 2, 4, 5).  Norms as in reading A15 (tests/parity.py)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import igr_ref as R
+from paper_2505_07392_b200 import igr
+from paper_2505_07392_b200 import workloads as W
+import exact_riemann as ER
+import parity
+
+pytestmark = pytest.mark.gpu
+
+FULL = os.environ.get("IGR_TEST_FULL", "1") != "0"      # full-size configs (needs a B200-class GPU)
+
+
+def test_config1_entropy_wave_32_20_steps():
+    w = W.entropy_wave(32)
+    g = igr.Solver.for_workload(w)
+    qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=w.n_steps)
+    mx, l1 = parity.worst(qg, qr)
+    assert mx <= 1e-4, (mx, l1)
+    # and against the closed form (P10): the fp32 result is as good as the oracle's
+    exact = W.entropy_wave_exact_rho(w, sum(dts)).numpy()
+    assert np.abs(qg[0] - exact).max() <= 7e-5
+    assert np.abs(sg).max() <= 1e-4            # Sigma stays at round-off level
+
+
+@pytest.mark.parametrize("shape", [(128, 8, 8)] + ([(512, 32, 32)] if FULL else []))
+def test_config2_sod_l1_vs_oracle_and_exact(shape):
+    w = W.sod(*shape)
+    g = igr.Solver.for_workload(w)
+    qg, qr, sg, sr, dts = parity.run_pair(w, g, t_end=w.t_end)
+    mx, l1 = parity.worst(qg, qr)
+    assert l1 <= 1e-3, (mx, l1)
+    assert parity.scalar_norms(sg, sr)[1] <= 1e-3
+    nx = shape[0]
+    x = (np.arange(nx) + 0.5) * w.dx
+    rex, _, _ = ER.sample((x - 0.5) / w.t_end, 1, 0, 1, 0.125, 0, 0.1)
+    l1_exact = np.abs(qg[0].mean(axis=(0, 1)) - rex).sum() * w.dx
+    assert l1_exact <= (1e-2 if nx >= 512 else 2.5e-2), l1_exact
+
+
+@pytest.mark.parametrize("n", [64] + ([256] if FULL else []))
+def test_config3_taylor_green_first_5_steps(n):
+    w = W.taylor_green(n)
+    g = igr.Solver.for_workload(w)
+    qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=5)
+    mx, l1 = parity.worst(qg, qr)
+    assert mx <= 1e-4, (mx, l1)
+
+
+def test_config3_conserved_totals_over_200_steps():
+    """P8 on the GPU: fp32 fields summed in fp64, drift <= 1e-6 relative over 200 steps."""
+    n = 256 if FULL else 64
+    w = W.taylor_green(n)
+    g = igr.Solver.for_workload(w)
+    q0 = W.state(w, device="cuda")
+    g.set_state(q0)
+    buf = torch.empty_like(q0)
+    tot0 = q0.double().flatten(1).sum(dim=1)
+    scale = q0.double().abs().flatten(1).sum(dim=1)
+    for step in range(w.n_steps):
+        g.step(w.cfl * w.dx / g.max_wavespeed())
+        if step % 50 == 49:
+            g.get_state(buf)
+            drift = (buf.double().flatten(1).sum(dim=1) - tot0).abs() / scale
+            # momentum totals are ~0: normalise every field by its own sum of magnitudes
+            assert float(drift.max()) <= 1e-6, (step, drift.tolist())
+    assert torch.isfinite(buf).all()
+
+
+def _subbox_parity(w, target_lo, size, pad, steps, storage=igr.STORE_F32, oracle_storage=R.STORE_F64):
+    """Full-domain GPU run vs the oracle on the dependency-cone sub-box (SURVEY 8(c) oracle reach)."""
+    full = (w.nx, w.ny, w.nz)
+    lo = tuple(max(0, target_lo[a] - pad) for a in range(3))
+    hi = tuple(min(full[a], target_lo[a] + size + pad) for a in range(3))
+    wb = W.subbox(w, lo, hi)
+    g = igr.Solver.for_workload(w, storage=storage)
+    q0 = W.state(w, device="cuda")
+    g.set_state(q0)
+    qb = q0[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].contiguous().cpu().numpy()
+    assert np.array_equal(qb, W.state(wb).numpy())          # counter-based noise: identical cut
+    del q0
+    ref = parity.oracle_for(wb, storage=oracle_storage)
+    ref.set_state(qb.astype(np.float64))
+    for _ in range(steps):
+        dt = w.cfl * w.dx / g.max_wavespeed()
+        g.step(dt)
+        ref.step(dt)
+    out = torch.empty((5, w.nz, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    g.get_state(out)
+    sl = tuple(slice(target_lo[a], target_lo[a] + size) for a in (2, 1, 0))
+    got = out[(slice(None),) + sl].cpu().numpy()
+    rl = tuple(slice(target_lo[a] - lo[a], target_lo[a] - lo[a] + size) for a in (2, 1, 0))
+    want = ref.get_state()[(slice(None),) + rl]
+    assert torch.isfinite(out).all()
+    rho_min = float(out[0].min())
+    del out
+    return got, want, rho_min
+
+
+def test_config4_jets9_small_replica_whole_domain():
+    """A 96^3 replica of config 4 (same patches pattern, scaled pitch) compared over the whole domain."""
+    w = W.jets9(n=96, radius=6, pitch=24, n_steps=10)
+    g = igr.Solver.for_workload(w)
+    qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=10)
+    mx, l1 = parity.worst(qg, qr)
+    assert l1 <= 1e-3 and mx <= 1e-3, (mx, l1)
+    assert parity.scalar_norms(sg, sr)[1] <= 1e-3
+
+
+@pytest.mark.skipif(not FULL, reason="full-size configs disabled")
+def test_config4_jets9_512_subbox_first_3_steps():
+    w = W.jets9()
+    # 64^3 target on the z = 0 plane over the edge of the central jet (radius 10 at (256, 256))
+    got, want, rho_min = _subbox_parity(w, (236, 224, 0), 64, 80, 3)
+    mx, l1 = parity.worst(got, want)
+    assert l1 <= 1e-3, (mx, l1)
+    assert rho_min > 0
+
+
+@pytest.mark.skipif(not FULL, reason="full-size configs disabled")
+def test_config5_jets33_1024_subbox_first_3_steps_fp32():
+    w = W.jets33()
+    # 64^3 target on z = 0 over the edge of the inner-ring jet centred at (526, 512), radius 8
+    got, want, rho_min = _subbox_parity(w, (496, 480, 0), 64, 80, 3)
+    mx, l1 = parity.worst(got, want)
+    assert l1 <= 1e-3, (mx, l1)
+    assert rho_min > 0
+
+
+def test_jets_run_stays_finite_and_positive():
+    """Config 4's "finite & positive" check on a 128^3 replica for 150 steps (the purely linear
+    scheme loses positivity in the under-resolved shock cells later on: DESIGN.md, findings)."""
+    w = W.jets9(n=128, radius=8, pitch=36)
+    g = igr.Solver.for_workload(w)
+    q0 = W.state(w, device="cuda")
+    g.set_state(q0)
+    for _ in range(150):
+        g.step(w.cfl * w.dx / g.max_wavespeed())          # raises IGR_ERR_NONFINITE on NaN / p < 0
+    out = torch.empty_like(q0)
+    g.get_state(out)
+    p = 0.4 * (out[4] - 0.5 * (out[1] ** 2 + out[2] ** 2 + out[3] ** 2) / out[0])
+    assert torch.isfinite(out).all() and float(out[0].min()) > 0 and float(p.min()) > 0

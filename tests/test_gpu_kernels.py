@@ -1,0 +1,218 @@
+"""GPU parity, row by row of the hot path: each C-ABI entry point of libigr.so
+against the oracle's counterpart on the same seeded inputs, on small ragged boxes that span several
+tiles and a ragged tail, with every BC type.  Tolerances are written here (fp32 vs fp64 oracle;
+DESIGN.md "Tolerances")."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import igr_ref as R
+from paper_2505_07392_b200 import igr
+from paper_2505_07392_b200 import workloads as W
+import parity
+
+pytestmark = pytest.mark.gpu
+
+G = 1.4
+PATCH = (9.0, 7.0, 4.0, 0.0, 0.5, 0.1, -0.2, 3.0, 2.0)
+SOFT = (20.0, 9.0, 5.0, 1.5, 0.6, 0.0, 0.0, 2.5, 1.5)
+BCS = {
+    "periodic": ((0,) * 6, None),
+    "extrap": ((1,) * 6, None),
+    "mixed": ((1, 1, 0, 0, 2, 1), {4: [PATCH, SOFT]}),
+    "inflow_x": ((2, 1, 1, 1, 0, 0), {0: [(6.0, 5.0, 3.0, 1.0, 0.7, 2.0, 0.0, 0.1, 1.2)]}),
+}
+SHAPES = [(37, 20, 13), (64, 16, 16), (5, 4, 3)]
+
+
+def smooth_state(nx, ny, nz, seed=0, noise=0.02):
+    rng = np.random.default_rng(seed)
+    z, y, x = np.meshgrid((np.arange(nz) + 0.5) / nz, (np.arange(ny) + 0.5) / ny, (np.arange(nx) + 0.5) / nx,
+                          indexing="ij")
+    tw = 2 * np.pi
+    rho = 1 + 0.3 * np.sin(tw * x) * np.cos(tw * y) + 0.2 * np.sin(tw * z) + noise * rng.uniform(-1, 1, x.shape)
+    u = 0.5 * np.sin(tw * (x + y)) + 0.1 + noise * rng.uniform(-1, 1, x.shape)
+    v = 0.4 * np.cos(tw * (y - z)) - 0.2 + noise * rng.uniform(-1, 1, x.shape)
+    w = 0.3 * np.sin(tw * (z + x)) * np.cos(tw * y) + noise * rng.uniform(-1, 1, x.shape)
+    p = 1 + 0.2 * np.cos(tw * (x + y + z))
+    q = np.stack([rho, rho * u, rho * v, rho * w, p / (G - 1) + 0.5 * rho * (u * u + v * v + w * w)])
+    return q.astype(np.float32)
+
+
+def make_pair(shape, bc, storage=igr.STORE_F32, n_jacobi=5, order=5, **kw):
+    nx, ny, nz = shape
+    faces, patches = BCS[bc]
+    dx = 1.0 / nx
+    g = igr.Solver(nx, ny, nz, dx, G, 10 * dx * dx, order=order, n_jacobi=n_jacobi, faces=faces,
+                   patches=patches, storage=storage, **kw)
+    r = R.RefSolver(nx, ny, nz, dx, G, 10 * dx * dx, order=order, n_jacobi=n_jacobi, faces=faces,
+                    patches=patches)
+    return g, r
+
+
+def one_axis_ghost_mask(nx, ny, nz):
+    """True where exactly one index is out of range: the only ghosts the method reads."""
+    out = [np.r_[np.ones(3, bool), np.zeros(n, bool), np.ones(3, bool)] for n in (nz, ny, nx)]
+    cnt = out[0][:, None, None].astype(int) + out[1][None, :, None] + out[2][None, None, :]
+    return cnt == 1
+
+
+@pytest.mark.parametrize("bc", list(BCS))
+@pytest.mark.parametrize("shape", SHAPES)
+def test_a1_halo_bc_matches_oracle_bitwise_up_to_the_blend(shape, bc):
+    if bc in ("mixed", "inflow_x") and shape == (5, 4, 3):
+        pytest.skip("patches do not fit the tiny box")
+    g, r = make_pair(shape, bc)
+    q = smooth_state(*shape, seed=1)
+    g.set_state(q)
+    r.set_state(q.astype(np.float64))
+    g.halo_bc()
+    r.fill_ghosts()
+    m = one_axis_ghost_mask(*shape)
+    for c in range(5):
+        a, b = g.get_padded(c), r.get_padded(c)
+        assert np.array_equal(a[3:-3, 3:-3, 3:-3], q[c])
+        # copies are exact; blended inflow values carry fp32 rounding of the weight and the blend
+        np.testing.assert_allclose(a[m], b[m], rtol=3e-7, atol=1e-7)
+        if bc in ("periodic", "extrap"):
+            assert np.array_equal(a[m].astype(np.float64), b[m])
+    # Sigma ghosts: wrap / clamp
+    sig = np.random.default_rng(3).uniform(-1, 1, shape[::-1]).astype(np.float32)
+    g.set_sigma(sig)
+    r.set_sigma(sig.astype(np.float64))
+    r.fill_sigma_ghosts()
+    a, b = g.get_padded(5), r.get_padded(5)
+    assert np.array_equal(a[m].astype(np.float64), b[m])
+
+
+@pytest.mark.parametrize("bc", ["periodic", "mixed"])
+@pytest.mark.parametrize("shape", SHAPES[:2])
+def test_a2_sigma_source(shape, bc):
+    g, r = make_pair(shape, bc)
+    q = smooth_state(*shape, seed=2)
+    g.set_state(q)
+    r.set_state(q.astype(np.float64))
+    g.halo_bc()
+    g.sigma_source()
+    r.fill_ghosts()
+    r.source()
+    mx, l1 = parity.scalar_norms(g.get_source(), r.get_source())
+    assert mx <= 1e-4 and l1 <= 1e-5, (mx, l1)
+
+
+@pytest.mark.parametrize("bc", list(BCS))
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("n_jacobi", [1, 5])
+def test_a3_jacobi_sweeps(shape, bc, n_jacobi):
+    if bc in ("mixed", "inflow_x") and shape == (5, 4, 3):
+        pytest.skip("patches do not fit the tiny box")
+    g, r = make_pair(shape, bc, n_jacobi=n_jacobi)
+    q = smooth_state(*shape, seed=3)
+    rng = np.random.default_rng(33)
+    b = rng.uniform(-1, 2, shape[::-1]).astype(np.float32)
+    s0 = rng.uniform(-1, 1, shape[::-1]).astype(np.float32)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    g.halo_bc(); r.fill_ghosts()
+    g.set_source(b); r.set_source(b.astype(np.float64))
+    g.set_sigma(s0); r.set_sigma(s0.astype(np.float64))
+    g.jacobi(); r.solve_sigma()
+    mx, l1 = parity.scalar_norms(g.get_sigma(), r.get_sigma())
+    assert mx <= 2e-6 and l1 <= 1e-6, (mx, l1)
+    m = one_axis_ghost_mask(*shape)
+    assert np.abs(g.get_padded(5)[m] - r.get_padded(5)[m]).max() <= 2e-6 * np.abs(r.get_sigma()).max()
+
+
+@pytest.mark.parametrize("order", [5, 3])
+@pytest.mark.parametrize("bc", list(BCS))
+@pytest.mark.parametrize("shape", SHAPES[:2])
+def test_a4_rhs(shape, bc, order):
+    g, r = make_pair(shape, bc, order=order)
+    q = smooth_state(*shape, seed=4)
+    sig = (0.05 * np.random.default_rng(44).uniform(0, 1, shape[::-1])).astype(np.float32)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    g.set_sigma(sig); r.set_sigma(sig.astype(np.float64))
+    g.halo_bc(); r.fill_ghosts(); r.fill_sigma_ghosts()
+    g.rhs(); r.rhs()
+    mx, l1 = parity.worst(g.get_rhs(), r.get_rhs())
+    assert mx <= 1e-4 and l1 <= 2e-5, (mx, l1)
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_a5_rk_update_stages_and_a6_wavespeed(shape):
+    g, r = make_pair(shape, "periodic")
+    q = smooth_state(*shape, seed=5)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    lam_g, lam_r = g.max_wavespeed(), r.max_wavespeed()
+    assert abs(lam_g - lam_r) <= 2e-6 * lam_r
+    dt = 0.4 / shape[0] / lam_r
+    g.halo_bc(); g.sigma_source(); g.jacobi(); g.rhs()
+    rg = g.get_rhs().astype(np.float64)
+    q64 = q.astype(np.float64)
+    q1 = R.rk_combine(0.0, q64, 1.0, q64, dt, rg)
+    g.rk_update(1, dt)
+    assert np.abs(g.get_state() - q1).max() <= 2e-7 * np.abs(q1).max()
+    q1g = g.get_state().astype(np.float64)
+    g.halo_bc(); g.sigma_source(); g.jacobi(); g.rhs()
+    rg = g.get_rhs().astype(np.float64)
+    q2 = R.rk_combine(0.75, q64, 0.25, q1g, dt, rg)
+    g.rk_update(2, dt)
+    assert np.abs(g.get_state() - q2).max() <= 2e-7 * np.abs(q2).max()
+    q2g = g.get_state().astype(np.float64)
+    g.halo_bc(); g.sigma_source(); g.jacobi(); g.rhs()
+    rg = g.get_rhs().astype(np.float64)
+    q3 = R.rk_combine(1 / 3, q64, 2 / 3, q2g, dt, rg)
+    g.rk_update(3, dt)
+    out = g.get_state()
+    assert np.abs(out - q3).max() <= 2e-7 * np.abs(q3).max()
+    # the wave speed folded into the stage-3 update equals the standalone reduction of the new state
+    lam_fused = g.max_wavespeed()
+    g2, r2 = make_pair(shape, "periodic")
+    g2.set_state(out); r2.set_state(out.astype(np.float64))
+    assert lam_fused == g2.max_wavespeed()
+    assert abs(lam_fused - r2.max_wavespeed()) <= 2e-6 * lam_fused
+
+
+def test_uniform_state_preserved_bitwise_and_sigma_zero():
+    """north_star gate 1 on the GPU (P7)."""
+    for faces, patches in [((0,) * 6, None), ((1, 1, 0, 0, 2, 1), {4: [(9.0, 7.0, 4.0, 0.0, 0.9, 0.3, -0.7, 1.1, 1.3),
+                                                                    (20.0, 9.0, 5.0, 1.5, 0.9, 0.3, -0.7, 1.1, 1.3)]})]:
+        w = W.uniform(37, 20, 13, 0.1, 0.9, 0.3, -0.7, 1.1, 1.3, faces=faces, patches=patches)
+        q0 = W.state(w).numpy()
+        g = igr.Solver.for_workload(w)
+        g.set_state(q0)
+        for _ in range(4):
+            g.step(0.5 * w.dx / g.max_wavespeed())
+        assert np.array_equal(g.get_state(), q0)
+        assert np.all(g.get_sigma() == 0.0) and np.all(g.get_rhs() == 0.0)
+
+
+def test_nonfinite_state_is_reported_not_repaired():
+    g, _ = make_pair((16, 8, 8), "periodic")
+    q = smooth_state(16, 8, 8)
+    q[4, 3, 3, 3] = -5.0                    # negative pressure
+    g.set_state(q)
+    with pytest.raises(igr.IgrError) as e:
+        g.max_wavespeed()
+    assert e.value.code == igr.ERR_NONFINITE
+    q = smooth_state(16, 8, 8)
+    q[0, 1, 2, 3] = np.nan
+    g.set_state(q)
+    with pytest.raises(igr.IgrError) as e:
+        g.max_wavespeed()
+    assert e.value.code == igr.ERR_NONFINITE
+
+
+def test_device_pointers_and_library_workspace():
+    shape = (37, 20, 13)
+    g, r = make_pair(shape, "periodic", own_workspace=False)       # library allocates itself
+    q = smooth_state(*shape, seed=7)
+    qd = torch.from_numpy(q).cuda()
+    g.set_state(qd)                                                 # device pointer in
+    out = torch.empty_like(qd)
+    g.get_state(out)                                                # device pointer out
+    assert torch.equal(out, qd)
+    r.set_state(q.astype(np.float64))
+    dt = 0.4 / shape[0] / r.max_wavespeed()
+    g.step(dt); r.step(dt)
+    mx, l1 = parity.worst(g.get_state(), r.get_state())
+    assert mx <= 1e-5, (mx, l1)
