@@ -358,9 +358,17 @@ __global__ void k_rhs_simple(Grid g, StagePtrs q, const T *__restrict__ sig, flo
         float acc[5] = { 0.f, 0.f, 0.f, 0.f, 0.f };
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
+            // both faces go through ONE instance of the flux code (no unrolling), so that the two
+            // cells sharing a face compute bitwise the same flux: exact conservation and exact
+            // preservation of uniform states (P7, P8)
             float Fp[5], Fm[5];
-            face_flux<T, ORDER>(d, q, sig, id, st[d], gamma, Fp);
-            face_flux<T, ORDER>(d, q, sig, id - st[d], st[d], gamma, Fm);
+#pragma unroll 1
+            for (int side = 0; side < 2; ++side) {
+                float F[5];
+                face_flux<T, ORDER>(d, q, sig, side ? id - st[d] : id, st[d], gamma, F);
+#pragma unroll
+                for (int c = 0; c < 5; ++c) { if (side) Fm[c] = F[c]; else Fp[c] = F[c]; }
+            }
 #pragma unroll
             for (int c = 0; c < 5; ++c) acc[c] -= (Fp[c] - Fm[c]) * inv_dx;
         }

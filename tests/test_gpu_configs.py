@@ -66,12 +66,12 @@ def test_config3_conserved_totals_over_200_steps():
     buf = torch.empty_like(q0)
     tot0 = q0.double().flatten(1).sum(dim=1)
     scale = q0.double().abs().flatten(1).sum(dim=1)
+    scale[1:4] = scale[1:4].sum()          # the momentum components share one denominator (A15)
     for step in range(w.n_steps):
         g.step(w.cfl * w.dx / g.max_wavespeed())
         if step % 50 == 49:
             g.get_state(buf)
             drift = (buf.double().flatten(1).sum(dim=1) - tot0).abs() / scale
-            # momentum totals are ~0: normalise every field by its own sum of magnitudes
             assert float(drift.max()) <= 1e-6, (step, drift.tolist())
     assert torch.isfinite(buf).all()
 
@@ -86,7 +86,9 @@ def _subbox_parity(w, target_lo, size, pad, steps, storage=igr.STORE_F32, oracle
     q0 = W.state(w, device="cuda")
     g.set_state(q0)
     qb = q0[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].contiguous().cpu().numpy()
-    assert np.array_equal(qb, W.state(wb).numpy())          # counter-based noise: identical cut
+    # the SAME array (a cut of the device-generated state) goes to the oracle; the sub-box
+    # generator reproduces it up to CPU/GPU libm differences (counter-based noise, A17)
+    np.testing.assert_allclose(qb, W.state(wb).numpy(), rtol=1e-6, atol=1e-7)
     del q0
     ref = parity.oracle_for(wb, storage=oracle_storage)
     ref.set_state(qb.astype(np.float64))
