@@ -23,8 +23,6 @@ sys.path.insert(0, ROOT)
 
 METRIC = "grind time ns/(cell*eqn*RHS), 3D IGR Euler SSP-RK3 step"
 UNIT = "ns/(cell*eqn*RHS)"
-# algorithmic HBM bytes per cell per launch of each row, fp32 storage
-ALG_BYTES_F32 = {"sigma_source": 20.0, "jacobi": 16.0, "rhs": 44.0, "rk_update": 73.3}
 
 
 def parse():
@@ -35,7 +33,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="jets33_1024")
     ap.add_argument("--storage", default="f32", choices=["f32", "f16", "bf16"])
-    ap.add_argument("--fused", type=int, default=0)
+    ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()

@@ -54,6 +54,9 @@ typedef enum {
 #define IGR_STORE_F16  1
 #define IGR_STORE_BF16 2
 
+#define IGR_VARIANT_TILED  0
+#define IGR_VARIANT_SIMPLE 1
+
 /* A circular inflow patch on a face.  (c0, c1) and radius are in CELL units on the face plane, the
  * transverse axes taken in the order x < y < z.  A ghost cell whose transverse centre (i+1/2, j+1/2)
  * lies at distance r from the centre gets, in all three ghost layers,
@@ -77,6 +80,9 @@ typedef struct {
     int32_t storage;       /* IGR_STORE_*                                                         */
     int32_t fused;         /* 0: one kernel per row of the hot path (source, Jacobi, RHS, update)  */
                            /* 1: RK update fused into the RHS kernel (one more state buffer)       */
+    int32_t variant;       /* IGR_VARIANT_TILED (default): TMA-staged tiled kernels;               */
+                           /* IGR_VARIANT_SIMPLE: one-thread-per-cell reference kernels (debugging) */
+    int32_t reserved;
     void   *stream;        /* cudaStream_t to run on (NULL: the legacy default stream)             */
     void   *workspace;     /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-B     */
     size_t  workspace_bytes; /* aligned, at least igr_workspace_bytes(); NULL: library allocates  */

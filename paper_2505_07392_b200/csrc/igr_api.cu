@@ -3,6 +3,7 @@
 // is done on the host except the fp64 evaluation of the inflow blend weights at creation.
 #include "../../include/igr.h"
 #include "igr_kernels.h"
+#include "igr_rhs_tile.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -55,7 +56,8 @@ Layout make_layout(const Grid &g, int storage, int fused)
 
 struct igr_solver {
     Grid g;
-    int storage = 0, fused = 0, order = 5, n_jacobi = 5;
+    int storage = 0, fused = 0, variant = 0, order = 5, n_jacobi = 5;
+    RhsTileMaps maps;
     double dx = 0, gamma = 0, alpha = 0;
     cudaStream_t stream = nullptr;
     char *base = nullptr;            // device memory (owned or caller's workspace)
@@ -252,6 +254,8 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     igr_solver *s = new igr_solver();
     s->storage = storage;
     s->fused = opt ? (opt->fused != 0) : 0;
+    s->variant = opt ? opt->variant : 0;
+    s->maps.valid = false;
     s->order = order; s->n_jacobi = n_jacobi;
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
     s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
@@ -285,6 +289,13 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->wave = (WaveResult *)p;
     int rc = build_inflow(s, bc);
     if (rc != IGR_OK) { igr_destroy(s); return rc; }
+    if (s->variant == IGR_VARIANT_TILED) {
+        const char *msg = "";
+        if (rhs_tile_make_maps(s->g, storage, s->st, L.n_state, s->sig, &s->maps, &msg) != 0) {
+            igr_destroy(s);
+            return IGR_ERR_CUDA;
+        }
+    }
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) { igr_destroy(s); return IGR_ERR_CUDA; }
     *out = s;
     return IGR_OK;
@@ -441,7 +452,14 @@ int igr_rhs(igr_solver *s)
     RowTimer t(s, 3, 1);
     RhsParams p;
     p.gamma = (float)s->gamma; p.inv_dx = (float)(1.0 / s->dx); p.order = s->order;
-    launch_rhs_simple(s->g, s->storage, s->st[s->cur], s->sig[s->sig_cur], s->r, p, s->stream);
+    if (s->variant == IGR_VARIANT_TILED) {
+        RhsTileArgs a = {};
+        for (int c = 0; c < 5; ++c) a.r[c] = s->r[c];
+        a.gamma = p.gamma; a.inv_dx = p.inv_dx; a.zc = 0;
+        launch_rhs_tile(s->g, s->storage, s->order, false, s->maps.q[s->cur], s->maps.sig[s->sig_cur], a, s->stream);
+    } else {
+        launch_rhs_simple(s->g, s->storage, s->st[s->cur], s->sig[s->sig_cur], s->r, p, s->stream);
+    }
     return finish(s, "igr_rhs");
 }
 
@@ -478,8 +496,28 @@ int igr_step(igr_solver *s, double dt)
         if ((rc = igr_halo_bc(s)) != IGR_OK) return rc;
         if ((rc = igr_sigma_source(s)) != IGR_OK) return rc;
         if ((rc = igr_jacobi(s)) != IGR_OK) return rc;
-        if ((rc = igr_rhs(s)) != IGR_OK) return rc;
-        if ((rc = igr_rk_update(s, stage, dt)) != IGR_OK) return rc;
+        if (s->fused && s->variant == IGR_VARIANT_TILED) {
+            // RHS + stage update + (stage 3) wave speed in one kernel: q^n = st[0] is only read
+            // pointwise, the sub-steps alternate st[1], st[2]; stage 3 writes st[0] in place.
+            RowTimer t(s, 3, 1);
+            RhsTileArgs a = {};
+            const int src = s->cur, dst = stage == 1 ? 1 : (stage == 2 ? 2 : 0);
+            for (int c = 0; c < 5; ++c) { a.qn[c] = s->st[0].f[c]; a.qout[c] = s->st[dst].f[c]; }
+            a.beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
+            a.dt = (float)dt; a.read_qn = stage != 1;
+            a.gamma = (float)s->gamma; a.inv_dx = (float)(1.0 / s->dx); a.zc = 0;
+            if (stage == 3) {
+                IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
+                a.wave = s->wave;
+            }
+            launch_rhs_tile(s->g, s->storage, s->order, true, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
+            s->cur = dst;
+            if (stage == 3) s->wave_valid = true;
+            if ((rc = finish(s, "igr_step (fused rhs)")) != IGR_OK) return rc;
+        } else {
+            if ((rc = igr_rhs(s)) != IGR_OK) return rc;
+            if ((rc = igr_rk_update(s, stage, dt)) != IGR_OK) return rc;
+        }
     }
     return IGR_OK;
 }

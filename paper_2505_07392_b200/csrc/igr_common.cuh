@@ -63,6 +63,24 @@ struct WaveResult {
     unsigned int nonfinite;   // != 0 if any cell produced a non-finite value
 };
 
+// max_d |u_d| + c of one cell with IEEE division and square root (rows a5/a6); sets `bad` instead of
+// returning a non-finite value
+__device__ __forceinline__ float wavespeed_of(float rho, float mx, float my, float mz, float E,
+                                              float gamma, bool &bad)
+{
+    // explicit rounding intrinsics: every inlined instance gives bitwise the same value
+    const float ir = __fdiv_rn(1.0f, rho);
+    float m2 = __fmul_rn(mx, mx);
+    m2 = __fmaf_rn(my, my, m2);
+    m2 = __fmaf_rn(mz, mz, m2);
+    const float p = __fmul_rn(gamma - 1.0f, __fmaf_rn(__fmul_rn(-0.5f, ir), m2, E));
+    const float c = __fsqrt_rn(__fmul_rn(__fmul_rn(gamma, p), ir));
+    const float v = __fmaf_rn(fmaxf(fabsf(mx), fmaxf(fabsf(my), fabsf(mz))), fabsf(ir), c);
+    // non-finite (NaN/Inf, or sqrt of a negative) is reported, never repaired (reading A10)
+    if (!(v <= 3.0e38f)) { bad = true; return 0.f; }
+    return v;
+}
+
 #define IGR_CUDA_OK(call)                                                                          \
     do {                                                                                           \
         cudaError_t e_ = (call);                                                                   \

@@ -420,17 +420,6 @@ __device__ __forceinline__ void block_reduce_wave(float v, bool bad, WaveResult 
     }
 }
 
-__device__ __forceinline__ float wavespeed_of(float rho, float mx, float my, float mz, float E,
-                                              float gamma, bool &bad)
-{
-    const float ir = 1.0f / rho;
-    const float p = (gamma - 1.0f) * (E - 0.5f * (mx * mx + my * my + mz * mz) * ir);
-    const float v = fmaxf(fabsf(mx), fmaxf(fabsf(my), fabsf(mz))) * fabsf(ir) + sqrtf(gamma * p * ir);
-    // non-finite (NaN/Inf, or sqrt of a negative) is reported, never repaired (reading A10)
-    if (!(v <= 3.0e38f)) { bad = true; return 0.f; }
-    return v;
-}
-
 template <typename T, bool WAVE>
 __global__ void k_rk_update(Grid g, StagePtrs qn, StagePtrs qs, StagePtrs qo, const float *r0,
                             const float *r1, const float *r2, const float *r3, const float *r4,
@@ -449,7 +438,7 @@ __global__ void k_rk_update(Grid g, StagePtrs qn, StagePtrs qs, StagePtrs qo, co
 #pragma unroll
         for (int c = 0; c < 5; ++c) {
             const float a = ldf((const T *)qn.f[c] + id), s = ldf((const T *)qs.f[c] + id);
-            o[c] = a + beta * ((s - a) + dt * rr[c][id]);
+            o[c] = __fmaf_rn(beta, __fmaf_rn(dt, rr[c][id], __fsub_rn(s, a)), a);
             stf((T *)qo.f[c] + id, o[c]);
             if (WAVE) o[c] = ldf((const T *)qo.f[c] + id);      // wave speed of the STORED state
         }

@@ -1,0 +1,534 @@
+// igr_rhs_tile.cu -- row a4 of the hot path for sm_100a: r = -div F^ from (q, Sigma), optionally fused
+// with the RK stage update (a5) and the wave-speed reduction (a6).
+//
+// Design: 2.5-D streaming.  A CTA owns a 32 x TY column of cells and marches
+// along z.  Whole xy-planes of the six fields (q[5] as one 4-D box, Sigma as a 3-D box) with their
+// 3-cell halos are staged into a 6-slot shared-memory ring by TMA (cp.async.bulk.tensor + mbarrier),
+// three planes ahead of use.  Each thread owns one (x, y) column: the z stencil lives in a sliding
+// register window (6 planes x 6 fields), the x and y stencils are read from the current plane in
+// shared memory.  Every face flux is computed exactly once per CTA: a thread computes the right (x+),
+// top (y+) and upper (z+) face of its cell; the x- face comes from the neighbouring lane by shuffle,
+// the y- face through shared memory, the z- face from the previous plane step (registers).  The
+// faces on the tile's low x and y edges are computed by two designated warps.  No atomics: each cell
+// differences its own six faces (gather form), so sums are deterministic and both cells adjacent to a
+// face see bitwise the same flux (conservation to round-off, uniform states preserved exactly).
+//
+// Arithmetic (same as k_rhs_simple): Alg. 1, eqs. 6-8 L119-L125.
+#include "igr_rhs_tile.cuh"
+
+#include <cstdio>
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
+
+namespace {
+
+constexpr int TX = 32;          // tile width = warp width
+constexpr int NSLOT = 6;        // ring slots (planes): 4 live + 2 in flight
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ float rcp_fast(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float sqrt_fast(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---- geometry of one ring slot for storage type T
+template <typename T, int TY>
+struct Tile {
+    static constexpr int HX = 16 / (int)sizeof(T);       // x halo of the box: 4 (fp32) / 8 (half) -> 16 B
+    static constexpr int BX = TX + 2 * HX;               // box extents
+    static constexpr int BY = TY + 6;
+    static constexpr int PE = BX * BY;                   // elements of one field in a plane
+    static constexpr int QBYTES = (5 * PE * (int)sizeof(T) + 127) / 128 * 128;
+    static constexpr int SBYTES = (PE * (int)sizeof(T) + 127) / 128 * 128;
+    static constexpr int SLOT = QBYTES + SBYTES;          // bytes per slot
+    static constexpr int TXBYTES = 6 * PE * (int)sizeof(T); // bytes one plane's two TMA loads deliver
+    static constexpr int AW = TX + 2;                     // width of the wave-speed arrays (halo 1)
+    static constexpr int RING = NSLOT * SLOT;
+    static constexpr int A_OFF = RING;                               // float ax[TY+2][AW], ay[TY+2][AW]
+    static constexpr int FY_OFF = A_OFF + 2 * (TY + 2) * AW * 4;     // float fy[5][TY][TX]
+    static constexpr int EX_OFF = FY_OFF + 5 * TY * TX * 4;          // float edge_x[5][TY]
+    static constexpr int EY_OFF = EX_OFF + 5 * TY * 4;               // float edge_y[5][TX]
+    static constexpr int BAR_OFF = (EY_OFF + 5 * TX * 4 + 7) / 8 * 8;
+    static constexpr int TOTAL = BAR_OFF + NSLOT * 8;
+};
+
+template <typename T> __device__ __forceinline__ float lds(const T *p);
+template <> __device__ __forceinline__ float lds<float>(const float *p) { return *p; }
+template <> __device__ __forceinline__ float lds<__half>(const __half *p) { return __half2float(*p); }
+template <> __device__ __forceinline__ float lds<__nv_bfloat16>(const __nv_bfloat16 *p) { return __bfloat162float(*p); }
+
+// ---- numerical flux at one face from the six stencil cells of the six fields.
+// t[f][s]: field f (rho, mx, my, mz, E, Sigma), stencil cell s = 0..5 <-> cells -2..3 about the face.
+// Returns G = 2 F^ = (F_L + F_R) - lambda (U_R - U_L); the factor 1/2 is folded into the divergence.
+// Written with explicit round-to-nearest intrinsics (never contracted or re-associated), so that every
+// inlined instance -- main path, edge warps, neighbouring CTAs -- produces bitwise the same flux from
+// the same inputs (conservation to round-off; uniform states preserved exactly, P7/P8).
+template <int ORDER>
+__device__ __forceinline__ void recon(const float t[6], float &l, float &r)
+{
+    if (ORDER == 5) {
+        l = __fmul_rn(2.f / 60.f, t[0]);
+        l = __fmaf_rn(-13.f / 60.f, t[1], l);
+        l = __fmaf_rn(47.f / 60.f, t[2], l);
+        l = __fmaf_rn(27.f / 60.f, t[3], l);
+        l = __fmaf_rn(-3.f / 60.f, t[4], l);
+        r = __fmul_rn(-3.f / 60.f, t[1]);
+        r = __fmaf_rn(27.f / 60.f, t[2], r);
+        r = __fmaf_rn(47.f / 60.f, t[3], r);
+        r = __fmaf_rn(-13.f / 60.f, t[4], r);
+        r = __fmaf_rn(2.f / 60.f, t[5], r);
+    } else {
+        l = __fmul_rn(-1.f / 6.f, t[1]);
+        l = __fmaf_rn(5.f / 6.f, t[2], l);
+        l = __fmaf_rn(2.f / 6.f, t[3], l);
+        r = __fmul_rn(2.f / 6.f, t[2]);
+        r = __fmaf_rn(5.f / 6.f, t[3], r);
+        r = __fmaf_rn(-1.f / 6.f, t[4], r);
+    }
+}
+
+// physical flux of one side along D from reconstructed conservative values U[0..4] and Sigma U[5]
+template <int D>
+__device__ __forceinline__ void side_flux2(const float U[6], float gm1, float F[5])
+{
+    const float ir = rcp_fast(U[0]);
+    const float ud = __fmul_rn(U[1 + D], ir);
+    float m2 = __fmul_rn(U[1], U[1]);
+    m2 = __fmaf_rn(U[2], U[2], m2);
+    m2 = __fmaf_rn(U[3], U[3], m2);
+    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, U[4]);     // E - |m|^2/(2 rho)
+    const float pt = __fmaf_rn(gm1, e, U[5]);                      // p + Sigma
+    F[0] = U[1 + D];
+    F[1] = (D == 0) ? __fmaf_rn(U[1], ud, pt) : __fmul_rn(U[1], ud);
+    F[2] = (D == 1) ? __fmaf_rn(U[2], ud, pt) : __fmul_rn(U[2], ud);
+    F[3] = (D == 2) ? __fmaf_rn(U[3], ud, pt) : __fmul_rn(U[3], ud);
+    F[4] = __fmul_rn(__fadd_rn(U[4], pt), ud);
+}
+
+template <int ORDER, int D>
+__device__ __forceinline__ void face_flux2(const float t[6][6], float lam, float gm1, float G[5])
+{
+    float L[6], R[6];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) recon<ORDER>(t[f], L[f], R[f]);
+    float FL[5], FR[5];
+    side_flux2<D>(L, gm1, FL);
+    side_flux2<D>(R, gm1, FR);
+#pragma unroll
+    for (int c = 0; c < 5; ++c)
+        G[c] = __fmaf_rn(-lam, __fsub_rn(R[c], L[c]), __fadd_rn(FL[c], FR[c]));
+}
+
+// cell-centred wave speeds |u_d| + c of one cell (reading A5); explicit intrinsics as above
+__device__ __forceinline__ void cell_speeds(float rho, float mx, float my, float mz, float E, float gamma,
+                                            float &ax, float &ay, float &az)
+{
+    const float ir = rcp_fast(rho);
+    float m2 = __fmul_rn(mx, mx);
+    m2 = __fmaf_rn(my, my, m2);
+    m2 = __fmaf_rn(mz, mz, m2);
+    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, E);
+    const float c = sqrt_fast(__fmul_rn(__fmul_rn(gamma, gamma - 1.0f), __fmul_rn(e, ir)));
+    ax = __fadd_rn(fabsf(__fmul_rn(mx, ir)), c);
+    ay = __fadd_rn(fabsf(__fmul_rn(my, ir)), c);
+    az = __fadd_rn(fabsf(__fmul_rn(mz, ir)), c);
+}
+
+}  // namespace
+
+// ======================================================================================= kernel
+template <typename T, int TY, int ORDER, bool FUSE>
+__global__ void __launch_bounds__(TX * TY, (TY <= 8) ? 2 : 1)
+k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap smap, Grid g,
+           RhsTileArgs a)
+{
+    using TL = Tile<T, TY>;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    float *A0 = reinterpret_cast<float *>(smem + TL::A_OFF);            // ax[(TY+2)][AW]
+    float *A1 = A0 + (TY + 2) * TL::AW;                                 // ay
+    float *FY = reinterpret_cast<float *>(smem + TL::FY_OFF);           // fy[5][TY][TX]
+    float *EX = reinterpret_cast<float *>(smem + TL::EX_OFF);           // edge_x[5][TY]
+    float *EY = reinterpret_cast<float *>(smem + TL::EY_OFF);           // edge_y[5][TX]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + TL::BAR_OFF);
+
+    const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5, warp = ty;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    const int kz0 = blockIdx.z * a.zc;
+    const int nkz = min(a.zc, g.nz - kz0);
+    const int i = x0 + tx, j = y0 + ty;
+    const bool valid = (i < g.nx) && (j < g.ny);
+    const float gm1 = a.gamma - 1.0f;
+    const float hdx = 0.5f * a.inv_dx;                 // G = 2 F^
+
+    // TMA coordinates of the box origin in the padded arrays (elements)
+    const int cx = g.gx + x0 - TL::HX, cy = y0, cz0 = kz0;       // plane p <-> padded z = kz0 + p
+    auto issue = [&](int p) {                                     // one elected thread
+        const int slot = p % NSLOT;
+        unsigned char *dst = smem + slot * TL::SLOT;
+        mbar_expect_tx(&full[slot], TL::TXBYTES);
+        tma_load_4d(dst, &qmap, cx, cy, cz0 + p, 0, &full[slot]);
+        tma_load_3d(dst + TL::QBYTES, &smap, cx, cy, cz0 + p, &full[slot]);
+    };
+    const int n_planes = nkz + 6;                                  // planes kz0-3 .. kz0+nkz+2
+    if (tid == 0) {
+        for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (int p = 0; p < NSLOT; ++p) issue(p);                  // n_planes >= 7 > NSLOT
+    }
+    __syncthreads();
+
+    const int own = (3 + ty) * TL::BX + TL::HX + tx;               // own cell inside a plane box
+    auto qbase = [&](int p) { return reinterpret_cast<const T *>(smem + (p % NSLOT) * TL::SLOT); };
+    auto sbase = [&](int p) { return reinterpret_cast<const T *>(smem + (p % NSLOT) * TL::SLOT + TL::QBYTES); };
+
+    // ---- prologue: window of planes p = 0..5 (cells kz0-3 .. kz0+2), flux of the face kz0-1/2
+    float W[6][6];                                                 // W[f][s]
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {
+        mbar_wait(&full[s], 0);
+        const T *qb = qbase(s) + own;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) W[f][s] = lds<T>(qb + f * TL::PE);
+        W[5][s] = lds<T>(sbase(s) + own);
+    }
+    float Gz_prev[5];
+    float ax_c, ay_c, az_c;
+    {
+        float bx, by, bz, az_m;
+        cell_speeds(W[0][2], W[1][2], W[2][2], W[3][2], W[4][2], a.gamma, bx, by, az_m);   // cell kz0-1
+        cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_c, ay_c, az_c); // cell kz0
+        face_flux2<ORDER, 2>(W, fmaxf(az_m, az_c), gm1, Gz_prev);
+        (void)bx; (void)by; (void)bz;
+    }
+#pragma unroll
+    for (int f = 0; f < 6; ++f) {
+#pragma unroll
+        for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];          // now cells kz0-2 .. kz0+2 in W[.][0..4]
+    }
+    __syncthreads();                                               // planes 0..2 are no longer needed
+    if (tid == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (int p = NSLOT; p < NSLOT + 3 && p < n_planes; ++p) issue(p);
+    }
+
+    float vmax = 0.f;
+    bool bad = false;
+
+    // ---- march: step t computes cell plane k = kz0 + t; current plane p = t + 3
+    for (int t = 0; t < nkz; ++t) {
+        const int pc = t + 3, pn = t + 6;
+        mbar_wait(&full[pn % NSLOT], (pn / NSLOT) & 1);
+        {
+            const T *qb = qbase(pn) + own;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) W[f][5] = lds<T>(qb + f * TL::PE);
+            W[5][5] = lds<T>(sbase(pn) + own);
+        }
+        // fused update: q^n of this cell is fetched now and consumed at the end of the step, so that
+        // the global-load latency hides behind the flux computation
+        float qn_pre[5];
+        const long long id = g.idx(i, j, kz0 + t);
+        if (FUSE) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c)
+                qn_pre[c] = (a.read_qn && valid) ? ldf(reinterpret_cast<const T *>(a.qn[c]) + id) : 0.f;
+        }
+        // wave speeds of the next cell (k+1) of this column; own values of plane k go to smem
+        float ax_n, ay_n, az_n;
+        cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_n, ay_n, az_n);
+        A0[(ty + 1) * TL::AW + tx + 1] = ax_c;
+        A1[(ty + 1) * TL::AW + tx + 1] = ay_c;
+        const T *qc = qbase(pc);
+        if (warp == 1 % TY) {
+            // halo cells of the wave-speed arrays: x-halo (tx = -1, 32) needs ax, y-halo (ty = -1, TY) ay
+            for (int h = tx; h < 2 * TY + 2 * TX; h += 32) {
+                int hx, hy;
+                if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
+                else { const int hh = h - 2 * TY; hy = (hh >= TX) ? TY : -1; hx = hh & (TX - 1); }
+                const T *c0 = qc + (3 + hy) * TL::BX + TL::HX + hx;
+                float hax, hay, haz;
+                cell_speeds(lds<T>(c0), lds<T>(c0 + TL::PE), lds<T>(c0 + 2 * TL::PE), lds<T>(c0 + 3 * TL::PE),
+                            lds<T>(c0 + 4 * TL::PE), a.gamma, hax, hay, haz);
+                A0[(hy + 1) * TL::AW + hx + 1] = hax;
+                A1[(hy + 1) * TL::AW + hx + 1] = hay;
+            }
+        }
+        __syncthreads();                                                           // sync 1
+
+        const T *sc = sbase(pc);
+        float Gx[5], Gy[5];
+        {   // x+ face of the own cell: cells i-2 .. i+3
+            float tp[6][6];
+            const T *qb = qc + own;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+#pragma unroll
+                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<T>(qb + f * TL::PE + (s - 2));
+            }
+#pragma unroll
+            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<T>(sc + own + (s - 2));
+            face_flux2<ORDER, 0>(tp, fmaxf(ax_c, A0[(ty + 1) * TL::AW + tx + 2]), gm1, Gx);
+        }
+        {   // y+ face: cells j-2 .. j+3
+            float tp[6][6];
+            const T *qb = qc + own;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+#pragma unroll
+                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<T>(qb + f * TL::PE + (s - 2) * TL::BX);
+            }
+#pragma unroll
+            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<T>(sc + own + (s - 2) * TL::BX);
+            face_flux2<ORDER, 1>(tp, fmaxf(ay_c, A1[(ty + 2) * TL::AW + tx + 1]), gm1, Gy);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) FY[(c * TY + ty) * TX + tx] = Gy[c];
+        }
+        if (warp == 2 % TY && tx < TY) {
+            // faces on the tile's low-x edge: between box columns HX-1 | HX of row tx
+            float tp[6][6], Ge[5];
+            const T *qb = qc + (3 + tx) * TL::BX + TL::HX - 1;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+#pragma unroll
+                for (int s = 0; s < 6; ++s) tp[f][s] = lds<T>(qb + f * TL::PE + (s - 2));
+            }
+#pragma unroll
+            for (int s = 0; s < 6; ++s) tp[5][s] = lds<T>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
+            face_flux2<ORDER, 0>(tp, fmaxf(A0[(tx + 1) * TL::AW + 0], A0[(tx + 1) * TL::AW + 1]), gm1, Ge);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) EX[c * TY + tx] = Ge[c];
+        }
+        if (warp == 3 % TY) {
+            // faces on the tile's low-y edge: between box rows 2 | 3 of column tx
+            float tp[6][6], Ge[5];
+            const T *qb = qc + 2 * TL::BX + TL::HX + tx;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+#pragma unroll
+                for (int s = 0; s < 6; ++s) tp[f][s] = lds<T>(qb + f * TL::PE + (s - 2) * TL::BX);
+            }
+#pragma unroll
+            for (int s = 0; s < 6; ++s) tp[5][s] = lds<T>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
+            face_flux2<ORDER, 1>(tp, fmaxf(A1[0 * TL::AW + tx + 1], A1[1 * TL::AW + tx + 1]), gm1, Ge);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
+        }
+        __syncthreads();                                                           // sync 2
+        if (tid == 0 && t + 9 < n_planes) {                      // slot of plane pc is free again
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            issue(t + 9);
+        }
+
+        // z+ face (cells k-2 .. k+3 of the own column), then the divergence
+        float Gz[5];
+        face_flux2<ORDER, 2>(W, fmaxf(az_c, az_n), gm1, Gz);
+        float r[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            float gxm = __shfl_up_sync(0xffffffffu, Gx[c], 1);
+            if (tx == 0) gxm = EX[c * TY + ty];
+            const float gym = (ty == 0) ? EY[c * TX + tx] : FY[(c * TY + ty - 1) * TX + tx];
+            // r = -(1/dx) sum_d (F^+ - F^-) with G = 2 F^
+            float acc = __fsub_rn(Gx[c], gxm);
+            acc = __fadd_rn(acc, __fsub_rn(Gy[c], gym));
+            acc = __fadd_rn(acc, __fsub_rn(Gz[c], Gz_prev[c]));
+            r[c] = __fmul_rn(-hdx, acc);
+            Gz_prev[c] = Gz[c];
+        }
+        if (valid) {
+            if (!FUSE) {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) a.r[c][id] = r[c];
+            } else {
+                float o[5];
+#pragma unroll
+                for (int c = 0; c < 5; ++c) {
+                    const float qs = W[c][2];
+                    const float qn = a.read_qn ? qn_pre[c] : qs;
+                    o[c] = __fmaf_rn(a.beta, __fmaf_rn(a.dt, r[c], __fsub_rn(qs, qn)), qn);
+                    stf(reinterpret_cast<T *>(a.qout[c]) + id, o[c]);
+                }
+                if (a.wave) {
+                    if (sizeof(T) < 4) {
+#pragma unroll
+                        for (int c = 0; c < 5; ++c) o[c] = ldf(reinterpret_cast<const T *>(a.qout[c]) + id);
+                    }
+                    vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], a.gamma, bad));
+                }
+            }
+        }
+        // slide the window
+#pragma unroll
+        for (int f = 0; f < 6; ++f) {
+#pragma unroll
+            for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];
+        }
+        ax_c = ax_n; ay_c = ay_n; az_c = az_n;
+    }
+
+    if (FUSE && a.wave) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+        const bool anybad = __any_sync(0xffffffffu, bad);
+        if (tx == 0) {
+            atomicMax(&a.wave->max_bits, __float_as_uint(vmax));
+            if (anybad) atomicOr(&a.wave->nonfinite, 1u);
+        }
+    }
+}
+
+// ======================================================================================= host
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+int tile_ty(const Grid &g) { return (g.ny >= 16 && (long long)g.nx * g.ny >= 128 * 128) ? 16 : 8; }
+
+}  // namespace
+
+int rhs_tile_default_zc(const Grid &g)
+{
+    // enough CTAs for ~4 waves of 148 SMs x (1 or 2) CTAs, chunks of at least 32 planes
+    const int ty = tile_ty(g);
+    const long long cols = (long long)((g.nx + TX - 1) / TX) * ((g.ny + ty - 1) / ty);
+    const long long want = 4LL * 148 * (ty == 8 ? 2 : 1);
+    long long nch = (want + cols - 1) / cols;
+    if (nch < 1) nch = 1;
+    int zc = (int)((g.nz + nch - 1) / nch);
+    if (zc < 32) zc = 32;
+    if (zc > g.nz) zc = g.nz;
+    return zc;
+}
+
+int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
+                       RhsTileMaps *out, const char **err)
+{
+    out->valid = false;
+    EncodeTiledFn enc = get_encode();
+    if (!enc) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
+    const size_t es = storage == 0 ? 4 : 2;
+    const CUtensorMapDataType dt = storage == 0 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                   : (storage == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
+    const int hx = 16 / (int)es, ty = tile_ty(g);
+    const cuuint32_t bx = TX + 2 * hx, by = ty + 6;
+    for (int b = 0; b < 3; ++b) {
+        const StagePtrs &s = st[b < n_state ? b : n_state - 1];
+        const cuuint64_t fstride = (cuuint64_t)((char *)s.f[1] - (char *)s.f[0]);
+        cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 5 };
+        cuuint64_t strides[3] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es, fstride };
+        cuuint32_t box[4] = { bx, by, 1, 5 }, estr[4] = { 1, 1, 1, 1 };
+        CUresult rc = enc(&out->q[b], dt, 4, s.f[0], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(q) failed"; return (int)rc; }
+    }
+    for (int b = 0; b < 2; ++b) {
+        cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz };
+        cuuint64_t strides[2] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es };
+        cuuint32_t box[3] = { bx, by, 1 }, estr[3] = { 1, 1, 1 };
+        CUresult rc = enc(&out->sig[b], dt, 3, sig[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(sigma) failed"; return (int)rc; }
+    }
+    out->valid = true;
+    return 0;
+}
+
+namespace {
+
+template <typename T, int TY, int ORDER, bool FUSE>
+void launch_one(const Grid &g, const CUtensorMap &qmap, const CUtensorMap &smap, RhsTileArgs a, cudaStream_t st)
+{
+    using TL = Tile<T, TY>;
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_rhs_tile<T, TY, ORDER, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, TL::TOTAL);
+        configured = true;
+    }
+    dim3 grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + a.zc - 1) / a.zc);
+    k_rhs_tile<T, TY, ORDER, FUSE><<<grid, TX * TY, TL::TOTAL, st>>>(qmap, smap, g, a);
+}
+
+template <typename T>
+void launch_t(const Grid &g, int order, bool fused, const CUtensorMap &qmap, const CUtensorMap &smap,
+              RhsTileArgs a, cudaStream_t st)
+{
+    const int ty = tile_ty(g);
+#define IGR_CASE(TYV, ORD, FU) launch_one<T, TYV, ORD, FU>(g, qmap, smap, a, st)
+    if (ty == 16) {
+        if (order == 5) { if (fused) IGR_CASE(16, 5, true); else IGR_CASE(16, 5, false); }
+        else { if (fused) IGR_CASE(16, 3, true); else IGR_CASE(16, 3, false); }
+    } else {
+        if (order == 5) { if (fused) IGR_CASE(8, 5, true); else IGR_CASE(8, 5, false); }
+        else { if (fused) IGR_CASE(8, 3, true); else IGR_CASE(8, 3, false); }
+    }
+#undef IGR_CASE
+}
+
+}  // namespace
+
+void launch_rhs_tile(const Grid &g, int storage, int order, bool fused, const CUtensorMap &qmap,
+                     const CUtensorMap &smap, RhsTileArgs a, cudaStream_t st)
+{
+    if (a.zc <= 0) a.zc = rhs_tile_default_zc(g);
+    if (storage == 0) launch_t<float>(g, order, fused, qmap, smap, a, st);
+    else if (storage == 1) launch_t<__half>(g, order, fused, qmap, smap, a, st);
+    else launch_t<__nv_bfloat16>(g, order, fused, qmap, smap, a, st);
+}

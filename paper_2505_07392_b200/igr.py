@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libigr.so")
 OK, ERR_ARG, ERR_BC, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
 BC_PERIODIC, BC_EXTRAP, BC_INFLOW = 0, 1, 2
 STORE_F32, STORE_F16, STORE_BF16 = 0, 1, 2
+VARIANT_TILED, VARIANT_SIMPLE = 0, 1
 _STATUS = {0: "IGR_OK", -1: "IGR_ERR_ARG", -2: "IGR_ERR_BC", -3: "IGR_ERR_ALLOC", -4: "IGR_ERR_CUDA",
            -5: "IGR_ERR_NONFINITE"}
 
@@ -43,7 +44,8 @@ class BC(C.Structure):
 
 
 class Options(C.Structure):
-    _fields_ = [("storage", C.c_int32), ("fused", C.c_int32), ("stream", C.c_void_p),
+    _fields_ = [("storage", C.c_int32), ("fused", C.c_int32), ("variant", C.c_int32),
+                ("reserved", C.c_int32), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -115,14 +117,14 @@ class Solver:
     """igr_create_ex / igr_destroy and the calls of include/igr.h on one solver object."""
 
     def __init__(self, nx, ny, nz, dx, gamma, alpha, order=5, n_jacobi=5, faces=(0,) * 6, patches=None,
-                 storage=STORE_F32, fused=0, device="cuda:0", own_workspace=True):
+                 storage=STORE_F32, fused=0, variant=VARIANT_TILED, device="cuda:0", own_workspace=True):
         L = lib()
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)
         self.device = torch.device(device)
         self._h = None
         opt = Options()
-        opt.storage, opt.fused = storage, fused
+        opt.storage, opt.fused, opt.variant = storage, fused, variant
         if not torch.cuda.is_available():
             raise IgrError(ERR_CUDA, "no CUDA device: libigr has no CPU fallback")
         torch.cuda.set_device(self.device)

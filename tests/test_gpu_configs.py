@@ -18,11 +18,14 @@ import parity
 pytestmark = pytest.mark.gpu
 
 FULL = os.environ.get("IGR_TEST_FULL", "1") != "0"      # full-size configs (needs a B200-class GPU)
+MODES = {"tiled": dict(), "tiled_fused": dict(fused=1), "simple": dict(variant=igr.VARIANT_SIMPLE)}
+BENCH_MODE = dict(fused=1)                               # the launch configuration bench.py times
 
 
-def test_config1_entropy_wave_32_20_steps():
+@pytest.mark.parametrize("mode", list(MODES))
+def test_config1_entropy_wave_32_20_steps(mode):
     w = W.entropy_wave(32)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **MODES[mode])
     qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=w.n_steps)
     mx, l1 = parity.worst(qg, qr)
     assert mx <= 1e-4, (mx, l1)
@@ -32,10 +35,11 @@ def test_config1_entropy_wave_32_20_steps():
     assert np.abs(sg).max() <= 1e-4            # Sigma stays at round-off level
 
 
-@pytest.mark.parametrize("shape", [(128, 8, 8)] + ([(512, 32, 32)] if FULL else []))
-def test_config2_sod_l1_vs_oracle_and_exact(shape):
+@pytest.mark.parametrize("shape,mode", [((128, 8, 8), m) for m in MODES] +
+                         ([((512, 32, 32), "tiled_fused")] if FULL else []))
+def test_config2_sod_l1_vs_oracle_and_exact(shape, mode):
     w = W.sod(*shape)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **MODES[mode])
     qg, qr, sg, sr, dts = parity.run_pair(w, g, t_end=w.t_end)
     mx, l1 = parity.worst(qg, qr)
     assert l1 <= 1e-3, (mx, l1)
@@ -47,10 +51,10 @@ def test_config2_sod_l1_vs_oracle_and_exact(shape):
     assert l1_exact <= (1e-2 if nx >= 512 else 2.5e-2), l1_exact
 
 
-@pytest.mark.parametrize("n", [64] + ([256] if FULL else []))
-def test_config3_taylor_green_first_5_steps(n):
+@pytest.mark.parametrize("n,mode", [(64, m) for m in MODES] + ([(256, "tiled_fused")] if FULL else []))
+def test_config3_taylor_green_first_5_steps(n, mode):
     w = W.taylor_green(n)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **MODES[mode])
     qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=5)
     mx, l1 = parity.worst(qg, qr)
     assert mx <= 1e-4, (mx, l1)
@@ -60,7 +64,7 @@ def test_config3_conserved_totals_over_200_steps():
     """P8 on the GPU: fp32 fields summed in fp64, drift <= 1e-6 relative over 200 steps."""
     n = 256 if FULL else 64
     w = W.taylor_green(n)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **BENCH_MODE)
     q0 = W.state(w, device="cuda")
     g.set_state(q0)
     buf = torch.empty_like(q0)
@@ -82,7 +86,7 @@ def _subbox_parity(w, target_lo, size, pad, steps, storage=igr.STORE_F32, oracle
     lo = tuple(max(0, target_lo[a] - pad) for a in range(3))
     hi = tuple(min(full[a], target_lo[a] + size + pad) for a in range(3))
     wb = W.subbox(w, lo, hi)
-    g = igr.Solver.for_workload(w, storage=storage)
+    g = igr.Solver.for_workload(w, storage=storage, **BENCH_MODE)
     q0 = W.state(w, device="cuda")
     g.set_state(q0)
     qb = q0[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].contiguous().cpu().numpy()
@@ -108,10 +112,11 @@ def _subbox_parity(w, target_lo, size, pad, steps, storage=igr.STORE_F32, oracle
     return got, want, rho_min
 
 
-def test_config4_jets9_small_replica_whole_domain():
+@pytest.mark.parametrize("mode", list(MODES))
+def test_config4_jets9_small_replica_whole_domain(mode):
     """A 96^3 replica of config 4 (same patches pattern, scaled pitch) compared over the whole domain."""
     w = W.jets9(n=96, radius=6, pitch=24, n_steps=10)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **MODES[mode])
     qg, qr, sg, sr, dts = parity.run_pair(w, g, n_steps=10)
     mx, l1 = parity.worst(qg, qr)
     assert l1 <= 1e-3 and mx <= 1e-3, (mx, l1)
@@ -142,7 +147,7 @@ def test_jets_run_stays_finite_and_positive():
     """Config 4's "finite & positive" check on a 128^3 replica for 150 steps (the purely linear
     scheme loses positivity in the under-resolved shock cells later on: DESIGN.md, findings)."""
     w = W.jets9(n=128, radius=8, pitch=36)
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **BENCH_MODE)
     q0 = W.state(w, device="cuda")
     g.set_state(q0)
     for _ in range(150):

@@ -122,11 +122,12 @@ def test_a3_jacobi_sweeps(shape, bc, n_jacobi):
     assert np.abs(g.get_padded(5)[m] - r.get_padded(5)[m]).max() <= 2e-6 * np.abs(r.get_sigma()).max()
 
 
+@pytest.mark.parametrize("variant", [igr.VARIANT_TILED, igr.VARIANT_SIMPLE])
 @pytest.mark.parametrize("order", [5, 3])
 @pytest.mark.parametrize("bc", list(BCS))
-@pytest.mark.parametrize("shape", SHAPES[:2])
-def test_a4_rhs(shape, bc, order):
-    g, r = make_pair(shape, bc, order=order)
+@pytest.mark.parametrize("shape", SHAPES[:2] + [(70, 33, 40)])
+def test_a4_rhs(shape, bc, order, variant):
+    g, r = make_pair(shape, bc, order=order, variant=variant)
     q = smooth_state(*shape, seed=4)
     sig = (0.05 * np.random.default_rng(44).uniform(0, 1, shape[::-1])).astype(np.float32)
     g.set_state(q); r.set_state(q.astype(np.float64))
@@ -172,8 +173,9 @@ def test_a5_rk_update_stages_and_a6_wavespeed(shape):
     assert abs(lam_fused - r2.max_wavespeed()) <= 2e-6 * lam_fused
 
 
+@pytest.mark.parametrize("mode", [dict(), dict(fused=1), dict(variant=igr.VARIANT_SIMPLE)])
 @pytest.mark.parametrize("case", ["periodic", "inflow"])
-def test_uniform_state_preserved_bitwise_and_sigma_zero(case):
+def test_uniform_state_preserved_bitwise_and_sigma_zero(case, mode):
     """north_star gate 1 on the GPU (P7).  The state is chosen exactly representable in fp32 so
     that the fixed patch state equals the interior bitwise."""
     st = (1.0, 0.5, -0.25, 1.0, 1.0)
@@ -181,18 +183,19 @@ def test_uniform_state_preserved_bitwise_and_sigma_zero(case):
         ((1, 1, 0, 0, 2, 1), {4: [(9.0, 7.0, 4.0, 0.0) + st, (20.0, 9.0, 5.0, 1.5) + st]})
     w = W.uniform(37, 20, 13, 0.1, *st, faces=faces, patches=patches)
     q0 = W.state(w).numpy()
-    g = igr.Solver.for_workload(w)
+    g = igr.Solver.for_workload(w, **mode)
     g.set_state(q0)
     for _ in range(4):
         g.step(0.5 * w.dx / g.max_wavespeed())
-    assert np.all(g.get_rhs() == 0.0)
+    if not mode.get("fused"):
+        assert np.all(g.get_rhs() == 0.0)
     assert np.all(g.get_sigma() == 0.0)
     assert np.array_equal(g.get_state(), q0)
     # a generic (not exactly representable) uniform state, periodic: still bitwise
     if case == "periodic":
         w = W.uniform(37, 20, 13, 0.1, 0.9, 0.3, -0.7, 1.1, 1.3)
         q0 = W.state(w).numpy()
-        g = igr.Solver.for_workload(w)
+        g = igr.Solver.for_workload(w, **mode)
         g.set_state(q0)
         for _ in range(4):
             g.step(0.5 * w.dx / g.max_wavespeed())
@@ -229,3 +232,38 @@ def test_device_pointers_and_library_workspace():
     g.step(dt); r.step(dt)
     mx, l1 = parity.worst(g.get_state(), r.get_state())
     assert mx <= 1e-5, (mx, l1)
+
+
+@pytest.mark.parametrize("shape", [(70, 33, 40), (64, 16, 16)])
+def test_fused_step_equals_unfused_step(shape):
+    """The RK update and wave speed fused into the RHS kernel give the same state as the separate
+    kernels (same arithmetic, so bitwise) and the same cached wave speed."""
+    q = smooth_state(*shape, seed=9)
+    out = []
+    for fused in (0, 1):
+        g, _ = make_pair(shape, "mixed", fused=fused)
+        g.set_state(q)
+        lam = []
+        for _ in range(3):
+            lam.append(g.max_wavespeed())
+            g.step(0.4 / shape[0] / lam[-1])
+        lam.append(g.max_wavespeed())
+        out.append((g.get_state(), g.get_sigma(), lam))
+    assert out[0][2] == out[1][2]
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.array_equal(out[0][1], out[1][1])
+
+
+def test_conservation_to_roundoff_tiled_periodic():
+    """P8 for the tiled kernel: every face flux is used with opposite signs by its two cells, also
+    across tile and chunk borders, so the totals move only by fp32 round-off of the update."""
+    shape = (96, 48, 80)
+    g, _ = make_pair(shape, "periodic", fused=1)
+    q = smooth_state(*shape, seed=10)
+    g.set_state(q)
+    tot0 = q.astype(np.float64).reshape(5, -1).sum(axis=1)
+    scale = np.abs(q).astype(np.float64).reshape(5, -1).sum(axis=1)
+    for _ in range(5):
+        g.step(0.4 / shape[0] / g.max_wavespeed())
+    tot = g.get_state().astype(np.float64).reshape(5, -1).sum(axis=1)
+    assert np.all(np.abs(tot - tot0) <= 2e-7 * scale), (tot - tot0) / scale
