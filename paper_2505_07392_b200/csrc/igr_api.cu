@@ -436,6 +436,18 @@ int igr_jacobi(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     const float k2 = (float)(s->alpha / (s->dx * s->dx));
+    if (s->variant == IGR_VARIANT_TILED) {
+        // temporally blocked: passes of up to 5 sweeps, each ONE read of rho, b, Sigma and one write
+        const int npass = (s->n_jacobi + 4) / 5;
+        RowTimer t(s, 2, npass + 1);
+        for (int left = s->n_jacobi; left > 0; left -= 5) {
+            launch_jacobi_blocked(s->g, s->storage, left < 5 ? left : 5, s->st[s->cur].f[0], s->b,
+                                  s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2, s->stream);
+            s->sig_cur = 1 - s->sig_cur;
+        }
+        launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);
+        return finish(s, "igr_jacobi");
+    }
     RowTimer t(s, 2, s->n_jacobi + 1);
     for (int it = 0; it < s->n_jacobi; ++it) {
         launch_jacobi_sweep(s->g, s->storage, s->st[s->cur].f[0], s->b, s->sig[s->sig_cur],

@@ -45,3 +45,7 @@ void launch_rk_update(const Grid &g, int storage, StagePtrs qn, StagePtrs qs, St
 // a6: wave = max_cells(max_d |u_d| + c), non-finite flag
 void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, WaveResult *wave,
                       cudaStream_t st);
+
+// a3 (blocked form): ns in 1..5 sweeps in ONE pass over HBM (igr_jacobi_blocked.cu); sig_in != sig_out
+void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, const float *b,
+                           const void *sig_in, void *sig_out, float k2, cudaStream_t st);

@@ -100,13 +100,16 @@ def test_a2_sigma_source(shape, bc):
     assert mx <= 1e-4 and l1 <= 1e-5, (mx, l1)
 
 
+@pytest.mark.parametrize("variant", [igr.VARIANT_TILED, igr.VARIANT_SIMPLE])
 @pytest.mark.parametrize("bc", list(BCS))
-@pytest.mark.parametrize("shape", SHAPES)
-@pytest.mark.parametrize("n_jacobi", [1, 5])
-def test_a3_jacobi_sweeps(shape, bc, n_jacobi):
+@pytest.mark.parametrize("shape", SHAPES + [(70, 33, 90)])
+@pytest.mark.parametrize("n_jacobi", [1, 3, 5, 7])
+def test_a3_jacobi_sweeps(shape, bc, n_jacobi, variant):
     if bc in ("mixed", "inflow_x") and shape == (5, 4, 3):
         pytest.skip("patches do not fit the tiny box")
-    g, r = make_pair(shape, bc, n_jacobi=n_jacobi)
+    if variant == igr.VARIANT_SIMPLE and n_jacobi in (3, 7):
+        pytest.skip("reference kernel: 1 and 5 sweeps suffice")
+    g, r = make_pair(shape, bc, n_jacobi=n_jacobi, variant=variant)
     q = smooth_state(*shape, seed=3)
     rng = np.random.default_rng(33)
     b = rng.uniform(-1, 2, shape[::-1]).astype(np.float32)
@@ -116,10 +119,11 @@ def test_a3_jacobi_sweeps(shape, bc, n_jacobi):
     g.set_source(b); r.set_source(b.astype(np.float64))
     g.set_sigma(s0); r.set_sigma(s0.astype(np.float64))
     g.jacobi(); r.solve_sigma()
+    # fp32 with approximate reciprocals (<= 1 ulp) in the seven coefficients of every sweep
     mx, l1 = parity.scalar_norms(g.get_sigma(), r.get_sigma())
-    assert mx <= 2e-6 and l1 <= 1e-6, (mx, l1)
+    assert mx <= 5e-6 and l1 <= 1e-6, (mx, l1)
     m = one_axis_ghost_mask(*shape)
-    assert np.abs(g.get_padded(5)[m] - r.get_padded(5)[m]).max() <= 2e-6 * np.abs(r.get_sigma()).max()
+    assert np.abs(g.get_padded(5)[m] - r.get_padded(5)[m]).max() <= 5e-6 * np.abs(r.get_sigma()).max()
 
 
 @pytest.mark.parametrize("variant", [igr.VARIANT_TILED, igr.VARIANT_SIMPLE])
