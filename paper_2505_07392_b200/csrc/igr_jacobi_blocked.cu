@@ -16,6 +16,8 @@
 // place of its outside neighbour.
 #include "igr_kernels.h"
 
+#include <type_traits>
+
 namespace {
 
 constexpr int R = 32;                       // region edge (threads per CTA = R*R)
@@ -37,8 +39,13 @@ __device__ __forceinline__ int rho_index(int i, int n, bool periodic)
     return min(max(i, -1), n);
 }
 
+constexpr int CPT = 2;                      // columns per thread: rows ry and ry + R/CPT of the region
+constexpr int NTHREADS = R * R / CPT;       // 512 threads x <= 128 registers: the whole pipeline state
+                                            // (7 coefficients x NS planes + 2 NS iterate values per
+                                            // column) stays in registers without spilling
+
 template <typename T, int NS>
-__global__ void __launch_bounds__(R * R, 1)
+__global__ void __launch_bounds__(NTHREADS, 1)
 k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bsrc, const T *__restrict__ sin,
                  T *__restrict__ sout, float k2, int zc)
 {
@@ -49,132 +56,183 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     float (*RHO)[PP] = reinterpret_cast<float (*)[PP]>(jb_smem);                       // [2][PP]
     float (*SP)[2][PP] = reinterpret_cast<float (*)[2][PP]>(jb_smem + 2 * PP);          // [NS][2][PP]
 
-    const int rx = threadIdx.x & 31, ry = threadIdx.x >> 5, pos = (ry + 1) * P + rx + 1;
-    const int gi = blockIdx.x * OT - NS + rx, gj = blockIdx.y * OT - NS + ry;
+    const int rx = threadIdx.x & 31, ry0 = threadIdx.x >> 5;
+    const int gi = blockIdx.x * OT - NS + rx;
     const int kz0 = blockIdx.z * zc, nkz = min(zc, g.nz - kz0);
     const bool per_x = g.bc[0] == 0, per_y = g.bc[2] == 0, per_z = g.bc[4] == 0;
-
-    // Store mask of this thread for the iterate planes.  Ghost values follow the BC index map at
-    // every sweep: a cell on a clamp boundary also writes its value into the neighbouring ghost
-    // position, and threads at positions outside a clamped domain do not store at all.
-    enum { ST_OWN = 1, ST_W = 2, ST_E = 4, ST_S = 8, ST_N = 16, ST_CORE = 32 };
-    int mask = 0;
-    {
-        const bool in_x = per_x || (gi >= 0 && gi < g.nx), in_y = per_y || (gj >= 0 && gj < g.ny);
-        if (in_x && in_y) {
-            mask |= ST_OWN;
-            if (!per_x && gi == 0) mask |= ST_W;
-            if (!per_x && gi == g.nx - 1) mask |= ST_E;
-            if (!per_y && gj == 0) mask |= ST_S;
-            if (!per_y && gj == g.ny - 1) mask |= ST_N;
-        }
-        if (rx >= NS && rx < R - NS && ry >= NS && ry < R - NS && gi < g.nx && gj < g.ny) mask |= ST_CORE;
-    }
-    auto put = [&](float *plane, float v) {
-        if (mask & ST_OWN) plane[pos] = v;
-        if (mask & ST_W) plane[pos - 1] = v;
-        if (mask & ST_E) plane[pos + 1] = v;
-        if (mask & ST_S) plane[pos - P] = v;
-        if (mask & ST_N) plane[pos + P] = v;
-    };
-
-    // element offsets fit 32 bits for every grid that fits the device memory
-    const unsigned off_r = (unsigned)(rho_index(gi, g.nx, per_x) + g.gx) +
-                           (unsigned)g.sy * (unsigned)(rho_index(gj, g.ny, per_y) + IGR_NG);
-    const unsigned off_m = (unsigned)(map_index(gi, g.nx, g.bc[0]) + g.gx) +
-                           (unsigned)g.sy * (unsigned)(map_index(gj, g.ny, g.bc[2]) + IGR_NG);
-    const unsigned off_o = (unsigned)(gi + g.gx) + (unsigned)g.sy * (unsigned)(gj + IGR_NG);
     const unsigned usz = (unsigned)g.sz;
 
-    auto load_plane = [&](int p, float &r0, float &b0, float &s0) {
-        const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
-        const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
-        r0 = ldf(rho + (off_r + zr));
-        b0 = bsrc[off_m + zm];
-        s0 = ldf(sin + (off_m + zm));
-    };
-
-    Coef C[NS];                              // ring: coefficient set of plane p lives in slot p mod NS
-    float below[NS], centre[NS];             // own column: level-l iterate at planes c-1, c (c = p1 - l)
+    // Ghost values of every iterate follow the BC index map at every sweep.  Periodic: the halo
+    // columns are wrapped real cells, recomputed.  Clamp: the ghost equals the nearest interior cell:
+    // a cell on a clamp boundary also writes its value into the neighbouring ghost position, and
+    // threads at positions outside a clamped domain do not store at all.
+    enum { ST_OWN = 1, ST_W = 2, ST_E = 4, ST_S = 8, ST_N = 16, ST_CORE = 32 };
+    int pos[CPT], mask[CPT];
+    unsigned off_r[CPT], off_m[CPT], off_o[CPT];     // element offsets fit 32 bits on any grid that fits
 #pragma unroll
-    for (int l = 0; l < NS; ++l) {
-        C[l].wxm = C[l].wxp = C[l].wym = C[l].wyp = C[l].wzp = C[l].dinv = C[l].b = 0.f;
-        below[l] = centre[l] = 0.f;
+    for (int cc = 0; cc < CPT; ++cc) {
+        const int ry = ry0 + cc * (R / CPT), gj = blockIdx.y * OT - NS + ry;
+        pos[cc] = (ry + 1) * P + rx + 1;
+        int m = 0;
+        const bool in_x = per_x || (gi >= 0 && gi < g.nx), in_y = per_y || (gj >= 0 && gj < g.ny);
+        if (in_x && in_y) {
+            m |= ST_OWN;
+            if (!per_x && gi == 0) m |= ST_W;
+            if (!per_x && gi == g.nx - 1) m |= ST_E;
+            if (!per_y && gj == 0) m |= ST_S;
+            if (!per_y && gj == g.ny - 1) m |= ST_N;
+        }
+        if (rx >= NS && rx < R - NS && ry >= NS && ry < R - NS && gi < g.nx && gj < g.ny) m |= ST_CORE;
+        mask[cc] = m;
+        off_r[cc] = (unsigned)(rho_index(gi, g.nx, per_x) + g.gx) +
+                    (unsigned)g.sy * (unsigned)(rho_index(gj, g.ny, per_y) + IGR_NG);
+        off_m[cc] = (unsigned)(map_index(gi, g.nx, g.bc[0]) + g.gx) +
+                    (unsigned)g.sy * (unsigned)(map_index(gj, g.ny, g.bc[2]) + IGR_NG);
+        off_o[cc] = (unsigned)(gi + g.gx) + (unsigned)g.sy * (unsigned)(gj + IGR_NG);
     }
-    float rho1 = 1.f, b1 = 0.f, wz_prev = 0.f;
-    for (int e = threadIdx.x; e < PP; e += R * R) {
+    // CTA-uniform: does this region touch a clamp boundary of the domain in x or y (or contain
+    // positions outside it)?  Interior CTAs take the variant of the loop body without any masks.
+    const int gi_lo = blockIdx.x * OT - NS, gj_lo = blockIdx.y * OT - NS;
+    const bool cta_edge = (!per_x && (gi_lo <= 0 || gi_lo + R >= g.nx)) || (!per_y && (gj_lo <= 0 || gj_lo + R >= g.ny));
+
+    Coef C[CPT][NS];                         // ring: coefficient set of plane p lives in slot p mod NS
+    float below[CPT][NS], centre[CPT][NS];   // own column: level-l iterate at planes c-1, c (c = p1 - l)
+    float rho1[CPT], b1[CPT], wz_prev[CPT], rn0[CPT], bn0[CPT], sn0[CPT];
+#pragma unroll
+    for (int cc = 0; cc < CPT; ++cc) {
+#pragma unroll
+        for (int l = 0; l < NS; ++l) {
+            C[cc][l].wxm = C[cc][l].wxp = C[cc][l].wym = C[cc][l].wyp = C[cc][l].wzp = 0.f;
+            C[cc][l].dinv = C[cc][l].b = 0.f;
+            below[cc][l] = centre[cc][l] = 0.f;
+        }
+        rho1[cc] = 1.f; b1[cc] = 0.f; wz_prev[cc] = 0.f;
+    }
+    for (int e = threadIdx.x; e < PP; e += NTHREADS) {
         RHO[0][e] = 1.f; RHO[1][e] = 1.f;
 #pragma unroll
         for (int l = 0; l < NS; ++l) { SP[l][0][e] = 0.f; SP[l][1][e] = 0.f; }
     }
 
+    auto load_plane = [&](int p) {
+        const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
+        const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
+#pragma unroll
+        for (int cc = 0; cc < CPT; ++cc) {
+            rn0[cc] = ldf(rho + (off_r[cc] + zr));
+            bn0[cc] = bsrc[off_m[cc] + zm];
+            sn0[cc] = ldf(sin + (off_m[cc] + zm));
+        }
+    };
+
+    // L2 prefetch of a plane three steps ahead (no registers): the register prefetch one step ahead
+    // then hits L2 instead of waiting for DRAM
+    auto prefetch_plane = [&](int p) {
+        const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
+        const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
+#pragma unroll
+        for (int cc = 0; cc < CPT; ++cc) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(rho + (off_r[cc] + zr)));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(bsrc + (off_m[cc] + zm)));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sin + (off_m[cc] + zm)));
+        }
+    };
+
     const int kfirst = kz0 - NS;             // first plane that enters; plane p <-> step p - kfirst
     const int nsteps = nkz + 2 * NS;         // output plane of step tau is kfirst + tau - NS
     const float k22 = 2.0f * k2;
-    float rn0, bn0, sn0;
-    load_plane(kfirst, rn0, bn0, sn0);
+    load_plane(kfirst);
+    prefetch_plane(kfirst + 1); prefetch_plane(kfirst + 2); prefetch_plane(kfirst + 3);
     __syncthreads();
 
-    for (int base = 0; base < nsteps; base += NS) {
+    // NS steps with compile-time ring slots; EDGE = false drops every boundary mask and select
+    auto group = [&](int base, auto edge_tag) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        auto put = [&](float *plane, int cc, float v) {
+            const int ps = pos[cc];
+            if (!EDGE) { plane[ps] = v; return; }
+            const int m = mask[cc];
+            if (m & ST_OWN) plane[ps] = v;
+            if (m & ST_W) plane[ps - 1] = v;
+            if (m & ST_E) plane[ps + 1] = v;
+            if (m & ST_S) plane[ps - P] = v;
+            if (m & ST_N) plane[ps + P] = v;
+        };
 #pragma unroll
         for (int u = 0; u < NS; ++u) {
             const int tau = base + u;
             const int p0 = kfirst + tau, p1 = p0 - 1;
-            const float rho0 = rn0, b0 = bn0, s0 = sn0;
-            if (tau + 1 < nsteps) load_plane(p0 + 1, rn0, bn0, sn0);        // prefetch the next plane
-            const int par0 = tau & 1, par1 = par0 ^ 1;                       // parity of planes p0 / p1
-            RHO[par0][pos] = rho0;
-            put(SP[0][par0], s0);
-
-            // ---- coefficients of plane p1 (its densities were stored in the previous step).
-            // Slot of plane p1 in the ring: (u - 1) mod NS (compile time); it held plane p1 - NS.
-            const int slot1 = (u + NS - 1) % NS;
-            const float wz_old = C[slot1].wzp;                               // W_z+ of plane p1 - NS
-            {
-                const float *rp = &RHO[par1][pos];
-                Coef c;
-                c.wxm = k22 * rcp_approx(rho1 + rp[-1]);
-                c.wxp = k22 * rcp_approx(rho1 + rp[1]);
-                c.wym = k22 * rcp_approx(rho1 + rp[-P]);
-                c.wyp = k22 * rcp_approx(rho1 + rp[P]);
-                c.wzp = k22 * rcp_approx(rho1 + rho0);
-                c.dinv = rcp_approx(rcp_approx(rho1) + ((c.wxm + c.wxp) + (c.wym + c.wyp) + (wz_prev + c.wzp)));
-                c.b = b1;
-                wz_prev = c.wzp;                                              // W_z- of the next plane
-                C[slot1] = c;
-            }
-
-            // ---- levels: level l+1 advances plane c = p1 - l
-            float above = s0;                                                 // level-0 iterate at plane p0
+            float rho0[CPT], b0[CPT], s0[CPT];
 #pragma unroll
-            for (int l = 0; l < NS; ++l) {
-                const int c = p1 - l;
-                const int slot = (u + 2 * NS - 1 - l) % NS;                   // slot of plane c
-                const int slot_m = (u + 2 * NS - 2 - l) % NS;                 // slot of plane c - 1
-                const float wzm = (l == NS - 1) ? wz_old : C[slot_m].wzp;
-                const float *sp = &SP[l][(par1 + l) & 1][pos];                // plane c of level l
-                const float ctr = centre[l];
-                const float dn = (!per_z && c == 0) ? ctr : below[l];
-                const float up = (!per_z && c == g.nz - 1) ? ctr : above;
-                float acc = C[slot].b;
-                acc = fmaf(C[slot].wxm, sp[-1], acc);
-                acc = fmaf(C[slot].wxp, sp[1], acc);
-                acc = fmaf(C[slot].wym, sp[-P], acc);
-                acc = fmaf(C[slot].wyp, sp[P], acc);
-                acc = fmaf(wzm, dn, acc);
-                acc = fmaf(C[slot].wzp, up, acc);
-                const float fresh = acc * C[slot].dinv;                       // level l+1 at plane c
-                below[l] = ctr;
-                centre[l] = above;
-                above = fresh;
-                if (l + 1 < NS) put(SP[l + 1][(par1 + l) & 1], fresh);       // plane c of level l+1
+            for (int cc = 0; cc < CPT; ++cc) { rho0[cc] = rn0[cc]; b0[cc] = bn0[cc]; s0[cc] = sn0[cc]; }
+            if (tau + 1 < nsteps) load_plane(p0 + 1);                        // prefetch the next plane
+            if (tau + 4 < nsteps) prefetch_plane(p0 + 4);
+            const int par0 = tau & 1, par1 = par0 ^ 1;                       // parity of planes p0 / p1
+            const int slot1 = (u + NS - 1) % NS;                              // ring slot of plane p1
+            const int ko = p0 - NS;                                           // output plane of this step
+            const bool out_ok = ko >= kz0 && ko < kz0 + nkz;
+#pragma unroll
+            for (int cc = 0; cc < CPT; ++cc) {
+                RHO[par0][pos[cc]] = rho0[cc];
+                put(SP[0][par0], cc, s0[cc]);
+
+                // ---- coefficients of plane p1 (its densities were stored in the previous step);
+                // the slot held plane p1 - NS, whose W_z+ the last level still needs
+                const float wz_old = C[cc][slot1].wzp;
+                {
+                    const float *rp = &RHO[par1][pos[cc]];
+                    const float r1 = rho1[cc];
+                    Coef c;
+                    c.wxm = k22 * rcp_approx(r1 + rp[-1]);
+                    c.wxp = k22 * rcp_approx(r1 + rp[1]);
+                    c.wym = k22 * rcp_approx(r1 + rp[-P]);
+                    c.wyp = k22 * rcp_approx(r1 + rp[P]);
+                    c.wzp = k22 * rcp_approx(r1 + rho0[cc]);
+                    c.dinv = rcp_approx(rcp_approx(r1) + ((c.wxm + c.wxp) + (c.wym + c.wyp) + (wz_prev[cc] + c.wzp)));
+                    c.b = b1[cc];
+                    wz_prev[cc] = c.wzp;                                      // W_z- of the next plane
+                    C[cc][slot1] = c;
+                }
+
+                // ---- levels: level l+1 advances plane c = p1 - l
+                float above = s0[cc];                                         // level-0 iterate at plane p0
+#pragma unroll
+                for (int l = 0; l < NS; ++l) {
+                    const int c = p1 - l;
+                    const int slot = (u + 2 * NS - 1 - l) % NS;               // slot of plane c
+                    const int slot_m = (u + 2 * NS - 2 - l) % NS;             // slot of plane c - 1
+                    const Coef &k = C[cc][slot];
+                    const float wzm = (l == NS - 1) ? wz_old : C[cc][slot_m].wzp;
+                    const float *sp = &SP[l][(par1 + l) & 1][pos[cc]];        // plane c of level l
+                    const float ctr = centre[cc][l];
+                    const float dn = (EDGE && !per_z && c == 0) ? ctr : below[cc][l];
+                    const float up = (EDGE && !per_z && c == g.nz - 1) ? ctr : above;
+                    float acc = k.b;
+                    acc = fmaf(k.wxm, sp[-1], acc);
+                    acc = fmaf(k.wxp, sp[1], acc);
+                    acc = fmaf(k.wym, sp[-P], acc);
+                    acc = fmaf(k.wyp, sp[P], acc);
+                    acc = fmaf(wzm, dn, acc);
+                    acc = fmaf(k.wzp, up, acc);
+                    const float fresh = acc * k.dinv;                         // level l+1 at plane c
+                    below[cc][l] = ctr;
+                    centre[cc][l] = above;
+                    above = fresh;
+                    if (l + 1 < NS) put(SP[l + 1][(par1 + l) & 1], cc, fresh);
+                }
+                // `above` now holds the level-NS iterate at plane p1 - (NS - 1) = p0 - NS
+                if ((mask[cc] & ST_CORE) && out_ok) stf(sout + (off_o[cc] + usz * (unsigned)(ko + IGR_NG)), above);
+                rho1[cc] = rho0[cc]; b1[cc] = b0[cc];
             }
-            // `above` now holds the level-NS iterate at plane p1 - (NS - 1) = p0 - NS
-            const int ko = p0 - NS;
-            if ((mask & ST_CORE) && ko >= kz0 && ko < kz0 + nkz) stf(sout + (off_o + usz * (unsigned)(ko + IGR_NG)), above);
-            rho1 = rho0; b1 = b0;
             __syncthreads();
         }
+    };
+    for (int base = 0; base < nsteps; base += NS) {
+        // planes touched by the levels of this group: kfirst + base - NS .. kfirst + base + NS - 1
+        const int plo = kfirst + base - NS, phi = kfirst + base + NS;
+        const bool z_edge = !per_z && ((plo <= 0 && phi >= 0) || (plo <= g.nz - 1 && phi >= g.nz - 1));
+        if (cta_edge || z_edge) group(base, std::true_type());
+        else group(base, std::false_type());
     }
 }
 
@@ -207,7 +265,7 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
                                  (2 + 2 * NSV) * (R + 2) * (R + 2) * 4);                                 \
             configured = true;                                                                           \
         }                                                                                                \
-        k_jacobi_blocked<T, NSV><<<grid, R * R, smem, st>>>(g, (const T *)rho, b, (const T *)sin,        \
+        k_jacobi_blocked<T, NSV><<<grid, NTHREADS, smem, st>>>(g, (const T *)rho, b, (const T *)sin,        \
                                                            (T *)sout, k2, zc);                           \
     } while (0)
     switch (ns) {

@@ -203,38 +203,36 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
 // footnote L252) with second-order central differences of the cell-centred velocity u = m/rho
 // (L132; Alg. 1).  G_ab = d u_a / d x_b.
 template <typename T>
-__global__ void k_source(Grid g, StagePtrs q, float *__restrict__ b, float alpha, float inv2dx)
+__global__ void __launch_bounds__(128) k_source(Grid g, StagePtrs q, float *__restrict__ b, float alpha, float inv2dx)
 {
+    // one thread per cell: x along the block, (j, k) from the grid -> no integer division
+    const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= g.nx) return;
     const T *rho = (const T *)q.f[0];
     const T *m[3] = { (const T *)q.f[1], (const T *)q.f[2], (const T *)q.f[3] };
-    const long long st[3] = { 1, g.sy, g.sz };
-    const long long n = (long long)g.nx * g.ny * g.nz;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
-         t += (long long)gridDim.x * blockDim.x) {
-        int i = (int)(t % g.nx); long long r = t / g.nx;
-        int j = (int)(r % g.ny), k = (int)(r / g.ny);
-        const long long id = g.idx(i, j, k);
-        float G[3][3];
+    const unsigned st[3] = { 1u, (unsigned)g.sy, (unsigned)g.sz };
+    const unsigned id = (unsigned)(i + g.gx) + st[1] * (unsigned)(j + IGR_NG) + st[2] * (unsigned)(k + IGR_NG);
+    float G[3][3];
 #pragma unroll
-        for (int bb = 0; bb < 3; ++bb) {
-            const long long ip = id + st[bb], im = id - st[bb];
-            const float rp = 1.0f / ldf(rho + ip), rm = 1.0f / ldf(rho + im);
+    for (int bb = 0; bb < 3; ++bb) {
+        const unsigned ip = id + st[bb], im = id - st[bb];
+        const float rp = __fdividef(1.0f, ldf(rho + ip)), rm = __fdividef(1.0f, ldf(rho + im));
 #pragma unroll
-            for (int a = 0; a < 3; ++a)
-                G[a][bb] = (ldf(m[a] + ip) * rp - ldf(m[a] + im) * rm) * inv2dx;
-        }
-        const float tr = G[0][0] + G[1][1] + G[2][2];
-        const float trsq = G[0][0] * G[0][0] + G[1][1] * G[1][1] + G[2][2] * G[2][2] +
-                           2.0f * (G[0][1] * G[1][0] + G[0][2] * G[2][0] + G[1][2] * G[2][1]);
-        b[id] = alpha * (trsq + tr * tr);
+        for (int a = 0; a < 3; ++a)
+            G[a][bb] = (ldf(m[a] + ip) * rp - ldf(m[a] + im) * rm) * inv2dx;
     }
+    const float tr = G[0][0] + G[1][1] + G[2][2];
+    const float trsq = G[0][0] * G[0][0] + G[1][1] * G[1][1] + G[2][2] * G[2][2] +
+                       2.0f * (G[0][1] * G[1][0] + G[0][2] * G[2][0] + G[1][2] * G[2][1]);
+    b[id] = alpha * (trsq + tr * tr);
 }
 
 void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
                    cudaStream_t st)
 {
-    long long n = (long long)g.nx * g.ny * g.nz;
-    DISPATCH_STORAGE(storage, k_source<T><<<blocks_for(n, 256), 256, 0, st>>>(g, q, b, alpha, inv2dx));
+    // grid.y / grid.z are limited to 65535: fine for every grid that fits the device
+    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
+    DISPATCH_STORAGE(storage, k_source<T><<<grid, 128, 0, st>>>(g, q, b, alpha, inv2dx));
 }
 
 // ------------------------------------------------------------------------------ a3: Jacobi sweep
