@@ -136,6 +136,24 @@ def alg_bytes(row, storage):
             "rk_update": (5 * (s + 4 + s) + 2 * 5 * (2 * s + 4 + s)) / 3.0}[row]
 
 
+def reduce_max(value, world, device="cpu"):
+    """Max over ranks of a host scalar (multi-GPU timing rule: the slowest rank counts)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_numbers(ms_step, cells_per_rank, world):
+    """Whole-job metric of `world` replicas that each advance `cells_per_rank` cells in ms_step (max
+    over ranks): grind time per (cell*eqn*RHS) of the job and aggregate cell updates per second."""
+    total = cells_per_rank * world
+    return {"grind_ns": ms_step * 1e6 / (total * 15), "cell_updates_per_s": total / (ms_step * 1e-3)}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -178,12 +196,10 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = g.kernel_launches() - l0
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = reduce_max(ms, world, dev)
     ms_step = ms / args.steps
-    grind = ms_step * 1e6 / (cells * 15)             # every rank does `cells`: per-job value is the same
+    job = job_numbers(ms_step, cells, world)
+    grind = job["grind_ns"]
 
     # per-row CUDA-event timing on the solver's stream (separate region, same state)
     nprof = max(1, min(args.steps, 5))
@@ -227,12 +243,9 @@ def run_ours(args):
             g.get_state(host)
         barrier()
         t_e2e = (time.perf_counter() - t0) / args.e2e_steps
-        if world > 1:
-            t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = reduce_max(t_e2e, world, dev)
         nbytes = 5 * cells * 4
-        e2e = {"value": t_e2e * 1e9 / (cells * 15), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": job_numbers(t_e2e * 1e3, cells, world)["grind_ns"], "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 8, "ms_per_step": t_e2e * 1e3, "pinned_host": pinned}
 
     out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -243,7 +256,7 @@ def run_ours(args):
                       "cfl": w.cfl, "parallelism": "replicas only" if world > 1 else "single GPU",
                       "l2": "inputs larger than L2 (no flush needed)" if cells * 4 > (126 << 20) else "inputs fit L2",
                       "wavespeed_query_every_step": True},
-           "cell_updates_per_s": world * cells / (ms_step * 1e-3),
+           "cell_updates_per_s": job["cell_updates_per_s"],
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w)
