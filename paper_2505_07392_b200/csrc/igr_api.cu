@@ -7,6 +7,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -438,10 +439,12 @@ int igr_jacobi(igr_solver *s)
     const float k2 = (float)(s->alpha / (s->dx * s->dx));
     if (s->variant == IGR_VARIANT_TILED) {
         // temporally blocked: passes of up to 5 sweeps, each ONE read of rho, b, Sigma and one write
-        const int npass = (s->n_jacobi + 4) / 5;
+        static int maxns = -1;                   // IGR_JACOBI_MAXNS=1..5: sweeps per blocked pass (tuning)
+        if (maxns < 0) { const char *e = getenv("IGR_JACOBI_MAXNS"); maxns = e ? atoi(e) : 5; if (maxns < 1 || maxns > 5) maxns = 5; }
+        const int npass = (s->n_jacobi + maxns - 1) / maxns;
         RowTimer t(s, 2, npass + 1);
-        for (int left = s->n_jacobi; left > 0; left -= 5) {
-            launch_jacobi_blocked(s->g, s->storage, left < 5 ? left : 5, s->st[s->cur].f[0], s->b,
+        for (int left = s->n_jacobi; left > 0; left -= maxns) {
+            launch_jacobi_blocked(s->g, s->storage, left < maxns ? left : maxns, s->st[s->cur].f[0], s->b,
                                   s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2, s->stream);
             s->sig_cur = 1 - s->sig_cur;
         }

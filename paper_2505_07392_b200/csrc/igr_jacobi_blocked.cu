@@ -40,6 +40,7 @@ __device__ __forceinline__ int rho_index(int i, int n, bool periodic)
 }
 
 constexpr int CPT = 2;                      // columns per thread: rows ry and ry + R/CPT of the region
+constexpr int PF = 3;                       // cp.async prefetch distance in planes (fp32 storage)
 constexpr int NTHREADS = R * R / CPT;       // 512 threads x <= 128 registers: the whole pipeline state
                                             // (7 coefficients x NS planes + 2 NS iterate values per
                                             // column) stays in registers without spilling
@@ -55,6 +56,10 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     extern __shared__ __align__(16) float jb_smem[];
     float (*RHO)[PP] = reinterpret_cast<float (*)[PP]>(jb_smem);                       // [2][PP]
     float (*SP)[2][PP] = reinterpret_cast<float (*)[2][PP]>(jb_smem + 2 * PP);          // [NS][2][PP]
+    // fp32 storage: incoming planes are staged by cp.async PF steps ahead (ring of PF + 1 stages of
+    // rho, b, Sigma for the R*R columns); each thread reads back only what it copied itself
+    float *STG = jb_smem + (2 + 2 * NS) * PP;                                           // [PF+1][3][R*R]
+    constexpr bool ASYNC = sizeof(T) == 4;
 
     const int rx = threadIdx.x & 31, ry0 = threadIdx.x >> 5;
     const int gi = blockIdx.x * OT - NS + rx;
@@ -114,7 +119,7 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
         for (int l = 0; l < NS; ++l) { SP[l][0][e] = 0.f; SP[l][1][e] = 0.f; }
     }
 
-    auto load_plane = [&](int p) {
+    auto load_plane = [&](int p) {               // register prefetch, one step ahead (half storage)
         const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
         const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
 #pragma unroll
@@ -124,25 +129,31 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
             sn0[cc] = ldf(sin + (off_m[cc] + zm));
         }
     };
-
-    // L2 prefetch of a plane three steps ahead (no registers): the register prefetch one step ahead
-    // then hits L2 instead of waiting for DRAM
-    auto prefetch_plane = [&](int p) {
+    auto cp4 = [](float *dst, const void *src) {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+    };
+    auto stage_plane = [&](int p, int stage) {   // asynchronous copy of plane p into a staging slot
         const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
         const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
+        float *st = STG + stage * 3 * R * R + threadIdx.x;
 #pragma unroll
         for (int cc = 0; cc < CPT; ++cc) {
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(rho + (off_r[cc] + zr)));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(bsrc + (off_m[cc] + zm)));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(sin + (off_m[cc] + zm)));
+            cp4(st + cc * NTHREADS, rho + (off_r[cc] + zr));
+            cp4(st + R * R + cc * NTHREADS, bsrc + (off_m[cc] + zm));
+            cp4(st + 2 * R * R + cc * NTHREADS, sin + (off_m[cc] + zm));
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
     const int kfirst = kz0 - NS;             // first plane that enters; plane p <-> step p - kfirst
     const int nsteps = nkz + 2 * NS;         // output plane of step tau is kfirst + tau - NS
     const float k22 = 2.0f * k2;
-    load_plane(kfirst);
-    prefetch_plane(kfirst + 1); prefetch_plane(kfirst + 2); prefetch_plane(kfirst + 3);
+    if (ASYNC) {
+#pragma unroll
+        for (int d = 0; d < PF; ++d) stage_plane(kfirst + d, d);
+    } else {
+        load_plane(kfirst);
+    }
     __syncthreads();
 
     // NS steps with compile-time ring slots; EDGE = false drops every boundary mask and select
@@ -163,10 +174,20 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
             const int tau = base + u;
             const int p0 = kfirst + tau, p1 = p0 - 1;
             float rho0[CPT], b0[CPT], s0[CPT];
+            if (ASYNC) {
+                // plane p0 was committed PF steps ago; keep PF groups in flight (empty groups at the end)
+                stage_plane(p0 + PF, (tau + PF) % (PF + 1));
+                asm volatile("cp.async.wait_group %0;" ::"n"(PF) : "memory");
+                const float *st = STG + (tau % (PF + 1)) * 3 * R * R + threadIdx.x;
 #pragma unroll
-            for (int cc = 0; cc < CPT; ++cc) { rho0[cc] = rn0[cc]; b0[cc] = bn0[cc]; s0[cc] = sn0[cc]; }
-            if (tau + 1 < nsteps) load_plane(p0 + 1);                        // prefetch the next plane
-            if (tau + 4 < nsteps) prefetch_plane(p0 + 4);
+                for (int cc = 0; cc < CPT; ++cc) {
+                    rho0[cc] = st[cc * NTHREADS]; b0[cc] = st[R * R + cc * NTHREADS]; s0[cc] = st[2 * R * R + cc * NTHREADS];
+                }
+            } else {
+#pragma unroll
+                for (int cc = 0; cc < CPT; ++cc) { rho0[cc] = rn0[cc]; b0[cc] = bn0[cc]; s0[cc] = sn0[cc]; }
+                if (tau + 1 < nsteps) load_plane(p0 + 1);                    // prefetch the next plane
+            }
             const int par0 = tau & 1, par1 = par0 ^ 1;                       // parity of planes p0 / p1
             const int slot1 = (u + NS - 1) % NS;                              // ring slot of plane p1
             const int ko = p0 - NS;                                           // output plane of this step
@@ -256,13 +277,13 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
 {
     const int ot = R - 2 * ns, zc = jacobi_blocked_zc(g, ns);
     dim3 grid((g.nx + ot - 1) / ot, (g.ny + ot - 1) / ot, (g.nz + zc - 1) / zc);
-    const int smem = (2 + 2 * ns) * (R + 2) * (R + 2) * 4;
+    const int smem = (2 + 2 * ns) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4;
 #define IGR_JB(NSV)                                                                                      \
     do {                                                                                                 \
         static bool configured = false;                                                                  \
         if (!configured) {                                                                               \
             cudaFuncSetAttribute(k_jacobi_blocked<T, NSV>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                                 (2 + 2 * NSV) * (R + 2) * (R + 2) * 4);                                 \
+                                 (2 + 2 * NSV) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4);      \
             configured = true;                                                                           \
         }                                                                                                \
         k_jacobi_blocked<T, NSV><<<grid, NTHREADS, smem, st>>>(g, (const T *)rho, b, (const T *)sin,        \

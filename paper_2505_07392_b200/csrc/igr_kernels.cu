@@ -202,37 +202,92 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
 // b = alpha ( tr((grad u)^2) + (tr grad u)^2 )  -- the side of eq. (9) that carries alpha (L127,
 // footnote L252) with second-order central differences of the cell-centred velocity u = m/rho
 // (L132; Alg. 1).  G_ab = d u_a / d x_b.
+// Streaming form: a CTA owns a 32 x 8 column of cells and marches along z.  Each cell's velocity is
+// computed once (one reciprocal per cell) and shared: in-plane neighbours through a triple-buffered
+// shared-memory plane with a one-cell halo, z neighbours in registers.  4 loads + 1 store per cell.
+constexpr int SRC_TX = 32, SRC_TY = 8, SRC_ZC = 64;
+
 template <typename T>
-__global__ void __launch_bounds__(128) k_source(Grid g, StagePtrs q, float *__restrict__ b, float alpha, float inv2dx)
+__global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q, float *__restrict__ b,
+                                                            float alpha, float inv2dx)
 {
-    // one thread per cell: x along the block, (j, k) from the grid -> no integer division
-    const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i >= g.nx) return;
+    constexpr int PW = SRC_TX + 2, PH = SRC_TY + 2, PN = PW * PH;
+    __shared__ float U[3][3][PN];                            // three plane buffers: one barrier per step
     const T *rho = (const T *)q.f[0];
     const T *m[3] = { (const T *)q.f[1], (const T *)q.f[2], (const T *)q.f[3] };
-    const unsigned st[3] = { 1u, (unsigned)g.sy, (unsigned)g.sz };
-    const unsigned id = (unsigned)(i + g.gx) + st[1] * (unsigned)(j + IGR_NG) + st[2] * (unsigned)(k + IGR_NG);
-    float G[3][3];
-#pragma unroll
-    for (int bb = 0; bb < 3; ++bb) {
-        const unsigned ip = id + st[bb], im = id - st[bb];
-        const float rp = __fdividef(1.0f, ldf(rho + ip)), rm = __fdividef(1.0f, ldf(rho + im));
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-            G[a][bb] = (ldf(m[a] + ip) * rp - ldf(m[a] + im) * rm) * inv2dx;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, tid = threadIdx.x;
+    const int x0 = blockIdx.x * SRC_TX, y0 = blockIdx.y * SRC_TY;
+    const int kz0 = blockIdx.z * SRC_ZC, nkz = min(SRC_ZC, g.nz - kz0);
+    // clamp the column into the padded array (columns beyond the domain compute unused values)
+    const int i = min(x0 + tx, g.nx), j = min(y0 + ty, g.ny);
+    const bool valid = (x0 + tx < g.nx) && (y0 + ty < g.ny);
+    const unsigned usz = (unsigned)g.sz;
+    const unsigned col = (unsigned)(i + g.gx) + (unsigned)g.sy * (unsigned)(j + IGR_NG);
+    const int own = (ty + 1) * PW + tx + 1;
+    // halo ring of the tile (2*32 + 2*8 cells): handled by the first 80 threads
+    int hpos = -1; unsigned hcol = 0;
+    if (tid < 2 * SRC_TX + 2 * SRC_TY) {
+        int hx, hy;
+        if (tid < 2 * SRC_TX) { hx = tid & 31; hy = (tid >> 5) ? SRC_TY : -1; }
+        else { const int t = tid - 2 * SRC_TX; hy = t & 7; hx = (t >> 3) ? SRC_TX : -1; }
+        const int hi = min(max(x0 + hx, -1), g.nx), hj = min(max(y0 + hy, -1), g.ny);
+        hpos = (hy + 1) * PW + hx + 1;
+        hcol = (unsigned)(hi + g.gx) + (unsigned)g.sy * (unsigned)(hj + IGR_NG);
     }
-    const float tr = G[0][0] + G[1][1] + G[2][2];
-    const float trsq = G[0][0] * G[0][0] + G[1][1] * G[1][1] + G[2][2] * G[2][2] +
-                       2.0f * (G[0][1] * G[1][0] + G[0][2] * G[2][0] + G[1][2] * G[2][1]);
-    b[id] = alpha * (trsq + tr * tr);
+    // raw loads of plane k (own column + halo cell) are issued one step before they are consumed
+    float rw[4], hw[4];
+    auto fetch = [&](int k) {
+        const unsigned zo = usz * (unsigned)(min(k, g.nz) + IGR_NG);
+        rw[0] = ldf(rho + col + zo); rw[1] = ldf(m[0] + col + zo); rw[2] = ldf(m[1] + col + zo); rw[3] = ldf(m[2] + col + zo);
+        if (hpos >= 0) {
+            hw[0] = ldf(rho + hcol + zo); hw[1] = ldf(m[0] + hcol + zo); hw[2] = ldf(m[1] + hcol + zo); hw[3] = ldf(m[2] + hcol + zo);
+        }
+    };
+    auto put_plane = [&](int buf, float &u, float &v, float &w) {          // fetched plane -> velocities
+        const float ir = __fdividef(1.0f, rw[0]);
+        u = rw[1] * ir; v = rw[2] * ir; w = rw[3] * ir;
+        U[buf][0][own] = u; U[buf][1][own] = v; U[buf][2][own] = w;
+        if (hpos >= 0) {
+            const float hr = __fdividef(1.0f, hw[0]);
+            U[buf][0][hpos] = hw[1] * hr; U[buf][1][hpos] = hw[2] * hr; U[buf][2][hpos] = hw[3] * hr;
+        }
+    };
+    float dn[3], ce[3], up[3];                               // own column at planes k-1, k, k+1
+    fetch(kz0 - 1);
+    {
+        const float ir = __fdividef(1.0f, rw[0]);
+        dn[0] = rw[1] * ir; dn[1] = rw[2] * ir; dn[2] = rw[3] * ir;
+    }
+    fetch(kz0);
+    put_plane(kz0 % 3, ce[0], ce[1], ce[2]);
+    fetch(kz0 + 1);
+    for (int t = 0; t < nkz; ++t) {
+        const int k = kz0 + t;
+        put_plane((k + 1) % 3, up[0], up[1], up[2]);         // next plane (the ghost plane at the top)
+        fetch(k + 2);                                        // lands during this step
+        __syncthreads();
+        const float (*P)[PN] = U[k % 3];
+        float G[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            G[a][0] = (P[a][own + 1] - P[a][own - 1]) * inv2dx;
+            G[a][1] = (P[a][own + PW] - P[a][own - PW]) * inv2dx;
+            G[a][2] = (up[a] - dn[a]) * inv2dx;
+        }
+        const float tr = G[0][0] + G[1][1] + G[2][2];
+        const float trsq = G[0][0] * G[0][0] + G[1][1] * G[1][1] + G[2][2] * G[2][2] +
+                           2.0f * (G[0][1] * G[1][0] + G[0][2] * G[2][0] + G[1][2] * G[2][1]);
+        if (valid) b[col + usz * (unsigned)(k + IGR_NG)] = alpha * (trsq + tr * tr);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { dn[a] = ce[a]; ce[a] = up[a]; }
+    }
 }
 
 void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
                    cudaStream_t st)
 {
-    // grid.y / grid.z are limited to 65535: fine for every grid that fits the device
-    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    DISPATCH_STORAGE(storage, k_source<T><<<grid, 128, 0, st>>>(g, q, b, alpha, inv2dx));
+    dim3 grid((g.nx + SRC_TX - 1) / SRC_TX, (g.ny + SRC_TY - 1) / SRC_TY, (g.nz + SRC_ZC - 1) / SRC_ZC);
+    DISPATCH_STORAGE(storage, k_source<T><<<grid, SRC_TX * SRC_TY, 0, st>>>(g, q, b, alpha, inv2dx));
 }
 
 // ------------------------------------------------------------------------------ a3: Jacobi sweep

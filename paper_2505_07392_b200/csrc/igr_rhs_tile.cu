@@ -17,6 +17,7 @@
 #include "igr_rhs_tile.cuh"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cuda_fp16.h>
 #include <cuda_bf16.h>
 
@@ -438,7 +439,13 @@ EncodeTiledFn get_encode()
     return fn;
 }
 
-int tile_ty(const Grid &g) { return (g.ny >= 16 && (long long)g.nx * g.ny >= 128 * 128) ? 16 : 8; }
+int tile_ty(const Grid &g)
+{
+    static int force = -1;                       // IGR_RHS_TY=8|16 overrides the heuristic (tuning)
+    if (force < 0) { const char *e = getenv("IGR_RHS_TY"); force = e ? atoi(e) : 0; }
+    if (force == 8 || force == 16) return force;
+    return 8;   // 2 CTAs of 256 threads per SM hide the per-plane barriers better than one of 512 (measured)
+}
 
 }  // namespace
 
