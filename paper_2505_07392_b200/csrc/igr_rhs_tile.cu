@@ -84,11 +84,13 @@ struct Tile {
     static constexpr int TXBYTES = 6 * PE * (int)sizeof(T); // bytes one plane's two TMA loads deliver
     static constexpr int AW = TX + 2;                     // width of the wave-speed arrays (halo 1)
     static constexpr int RING = NSLOT * SLOT;
-    static constexpr int A_OFF = RING;                               // float ax[TY+2][AW], ay[TY+2][AW]
-    static constexpr int FY_OFF = A_OFF + 2 * (TY + 2) * AW * 4;     // float fy[5][TY][TX]
-    static constexpr int EX_OFF = FY_OFF + 5 * TY * TX * 4;          // float edge_x[5][TY]
-    static constexpr int EY_OFF = EX_OFF + 5 * TY * 4;               // float edge_y[5][TX]
-    static constexpr int BAR_OFF = (EY_OFF + 5 * TX * 4 + 7) / 8 * 8;
+    // everything below is double-buffered by plane / step parity: one __syncthreads per plane
+    static constexpr int A_N = (TY + 2) * AW;                        // floats of one wave-speed array
+    static constexpr int A_OFF = RING;                               // float [2][ax | ay][A_N]
+    static constexpr int FY_OFF = A_OFF + 2 * 2 * A_N * 4;           // float [2][5][TY][TX]
+    static constexpr int EX_OFF = FY_OFF + 2 * 5 * TY * TX * 4;      // float [2][5][TY]
+    static constexpr int EY_OFF = EX_OFF + 2 * 5 * TY * 4;           // float [2][5][TX]
+    static constexpr int BAR_OFF = (EY_OFF + 2 * 5 * TX * 4 + 7) / 8 * 8;
     static constexpr int TOTAL = BAR_OFF + NSLOT * 8;
 };
 
@@ -184,11 +186,10 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 {
     using TL = Tile<T, TY>;
     extern __shared__ __align__(1024) unsigned char smem[];
-    float *A0 = reinterpret_cast<float *>(smem + TL::A_OFF);            // ax[(TY+2)][AW]
-    float *A1 = A0 + (TY + 2) * TL::AW;                                 // ay
-    float *FY = reinterpret_cast<float *>(smem + TL::FY_OFF);           // fy[5][TY][TX]
-    float *EX = reinterpret_cast<float *>(smem + TL::EX_OFF);           // edge_x[5][TY]
-    float *EY = reinterpret_cast<float *>(smem + TL::EY_OFF);           // edge_y[5][TX]
+    float *Abase = reinterpret_cast<float *>(smem + TL::A_OFF);         // [2][ax | ay][(TY+2)][AW]
+    float *FYbase = reinterpret_cast<float *>(smem + TL::FY_OFF);       // [2][5][TY][TX]
+    float *EXbase = reinterpret_cast<float *>(smem + TL::EX_OFF);       // [2][5][TY]
+    float *EYbase = reinterpret_cast<float *>(smem + TL::EY_OFF);       // [2][5][TX]
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + TL::BAR_OFF);
 
     const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5, warp = ty;
@@ -246,6 +247,29 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 #pragma unroll
         for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];          // now cells kz0-2 .. kz0+2 in W[.][0..4]
     }
+    // cell-centred wave speeds |u_d| + c of plane p (own cells from registers, the halo ring of the
+    // tile from the ring slot, by warp 1) into the buffer of that plane's parity
+    auto put_speeds = [&](int p, float oax, float oay) {
+        float *A0 = Abase + (p & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
+        A0[(ty + 1) * TL::AW + tx + 1] = oax;
+        A1[(ty + 1) * TL::AW + tx + 1] = oay;
+        if (warp == 1 % TY) {
+            // x-halo (tx = -1, 32) needs ax, y-halo (ty = -1, TY) needs ay
+            const T *qp = qbase(p);
+            for (int h = tx; h < 2 * TY + 2 * TX; h += 32) {
+                int hx, hy;
+                if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
+                else { const int hh = h - 2 * TY; hy = (hh >= TX) ? TY : -1; hx = hh & (TX - 1); }
+                const T *c0 = qp + (3 + hy) * TL::BX + TL::HX + hx;
+                float hax, hay, haz;
+                cell_speeds(lds<T>(c0), lds<T>(c0 + TL::PE), lds<T>(c0 + 2 * TL::PE), lds<T>(c0 + 3 * TL::PE),
+                            lds<T>(c0 + 4 * TL::PE), a.gamma, hax, hay, haz);
+                A0[(hy + 1) * TL::AW + hx + 1] = hax;
+                A1[(hy + 1) * TL::AW + hx + 1] = hay;
+            }
+        }
+    };
+    put_speeds(3, ax_c, ay_c);                                     // plane of the first cell layer kz0
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -274,27 +298,13 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             for (int c = 0; c < 5; ++c)
                 qn_pre[c] = (a.read_qn && valid) ? ldf(reinterpret_cast<const T *>(a.qn[c]) + id) : 0.f;
         }
-        // wave speeds of the next cell (k+1) of this column; own values of plane k go to smem
+        // wave speeds of the next cell (k+1) of this column, published for the next step
         float ax_n, ay_n, az_n;
         cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_n, ay_n, az_n);
-        A0[(ty + 1) * TL::AW + tx + 1] = ax_c;
-        A1[(ty + 1) * TL::AW + tx + 1] = ay_c;
+        put_speeds(pc + 1, ax_n, ay_n);                           // read in the next step (after the barrier)
         const T *qc = qbase(pc);
-        if (warp == 1 % TY) {
-            // halo cells of the wave-speed arrays: x-halo (tx = -1, 32) needs ax, y-halo (ty = -1, TY) ay
-            for (int h = tx; h < 2 * TY + 2 * TX; h += 32) {
-                int hx, hy;
-                if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
-                else { const int hh = h - 2 * TY; hy = (hh >= TX) ? TY : -1; hx = hh & (TX - 1); }
-                const T *c0 = qc + (3 + hy) * TL::BX + TL::HX + hx;
-                float hax, hay, haz;
-                cell_speeds(lds<T>(c0), lds<T>(c0 + TL::PE), lds<T>(c0 + 2 * TL::PE), lds<T>(c0 + 3 * TL::PE),
-                            lds<T>(c0 + 4 * TL::PE), a.gamma, hax, hay, haz);
-                A0[(hy + 1) * TL::AW + hx + 1] = hax;
-                A1[(hy + 1) * TL::AW + hx + 1] = hay;
-            }
-        }
-        __syncthreads();                                                           // sync 1
+        const float *A0 = Abase + (pc & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
+        float *FY = FYbase + (t & 1) * 5 * TY * TX, *EX = EXbase + (t & 1) * 5 * TY, *EY = EYbase + (t & 1) * 5 * TX;
 
         const T *sc = sbase(pc);
         float Gx[5], Gy[5];
@@ -354,7 +364,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 #pragma unroll
             for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
         }
-        __syncthreads();                                                           // sync 2
+        __syncthreads();                                   // the only barrier of the step
         if (tid == 0 && t + 9 < n_planes) {                      // slot of plane pc is free again
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             issue(t + 9);
