@@ -203,8 +203,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 
     // TMA coordinates of the box origin in the padded arrays (elements)
     const int cx = g.gx + x0 - TL::HX, cy = y0, cz0 = kz0;       // plane p <-> padded z = kz0 + p
-    auto issue = [&](int p) {                                     // one elected thread
-        const int slot = p % NSLOT;
+    auto issue = [&](int p, int slot) {                           // one elected thread; slot = p mod NSLOT
         unsigned char *dst = smem + slot * TL::SLOT;
         mbar_expect_tx(&full[slot], TL::TXBYTES);
         tma_load_4d(dst, &qmap, cx, cy, cz0 + p, 0, &full[slot]);
@@ -215,13 +214,14 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        for (int p = 0; p < NSLOT; ++p) issue(p);                  // n_planes >= 7 > NSLOT
+        for (int p = 0; p < NSLOT; ++p) issue(p, p);               // n_planes >= 7 > NSLOT
     }
     __syncthreads();
 
     const int own = (3 + ty) * TL::BX + TL::HX + tx;               // own cell inside a plane box
-    auto qbase = [&](int p) { return reinterpret_cast<const T *>(smem + (p % NSLOT) * TL::SLOT); };
-    auto sbase = [&](int p) { return reinterpret_cast<const T *>(smem + (p % NSLOT) * TL::SLOT + TL::QBYTES); };
+    // slot = plane index mod NSLOT; the march keeps the slot indices as wrapping counters (no division)
+    auto qbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT); };
+    auto sbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT + TL::QBYTES); };
 
     // ---- prologue: window of planes p = 0..5 (cells kz0-3 .. kz0+2), flux of the face kz0-1/2
     float W[6][6];                                                 // W[f][s]
@@ -249,13 +249,13 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     }
     // cell-centred wave speeds |u_d| + c of plane p (own cells from registers, the halo ring of the
     // tile from the ring slot, by warp 1) into the buffer of that plane's parity
-    auto put_speeds = [&](int p, float oax, float oay) {
+    auto put_speeds = [&](int p, int slot, float oax, float oay) {
         float *A0 = Abase + (p & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
         A0[(ty + 1) * TL::AW + tx + 1] = oax;
         A1[(ty + 1) * TL::AW + tx + 1] = oay;
         if (warp == 1 % TY) {
             // x-halo (tx = -1, 32) needs ax, y-halo (ty = -1, TY) needs ay
-            const T *qp = qbase(p);
+            const T *qp = qbase(slot);
             for (int h = tx; h < 2 * TY + 2 * TX; h += 32) {
                 int hx, hy;
                 if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
@@ -269,25 +269,27 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             }
         }
     };
-    put_speeds(3, ax_c, ay_c);                                     // plane of the first cell layer kz0
+    put_speeds(3, 3, ax_c, ay_c);                                  // plane of the first cell layer kz0
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        for (int p = NSLOT; p < NSLOT + 3 && p < n_planes; ++p) issue(p);
+        for (int p = NSLOT; p < NSLOT + 3 && p < n_planes; ++p) issue(p, p - NSLOT);
     }
 
     float vmax = 0.f;
     bool bad = false;
 
     // ---- march: step t computes cell plane k = kz0 + t; current plane p = t + 3
+    int slot_c = 3, slot_n = 0, phase_n = 1;                      // slots of planes t + 3 and t + 6
     for (int t = 0; t < nkz; ++t) {
-        const int pc = t + 3, pn = t + 6;
-        mbar_wait(&full[pn % NSLOT], (pn / NSLOT) & 1);
+        const int pc = t + 3;
+        const int slot_c1 = (slot_c == NSLOT - 1) ? 0 : slot_c + 1;  // slot of plane pc + 1
+        mbar_wait(&full[slot_n], phase_n);
         {
-            const T *qb = qbase(pn) + own;
+            const T *qb = qbase(slot_n) + own;
 #pragma unroll
             for (int f = 0; f < 5; ++f) W[f][5] = lds<T>(qb + f * TL::PE);
-            W[5][5] = lds<T>(sbase(pn) + own);
+            W[5][5] = lds<T>(sbase(slot_n) + own);
         }
         // fused update: q^n of this cell is fetched now and consumed at the end of the step, so that
         // the global-load latency hides behind the flux computation
@@ -301,12 +303,12 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         // wave speeds of the next cell (k+1) of this column, published for the next step
         float ax_n, ay_n, az_n;
         cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_n, ay_n, az_n);
-        put_speeds(pc + 1, ax_n, ay_n);                           // read in the next step (after the barrier)
-        const T *qc = qbase(pc);
+        put_speeds(pc + 1, slot_c1, ax_n, ay_n);                  // read in the next step (after the barrier)
+        const T *qc = qbase(slot_c);
         const float *A0 = Abase + (pc & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
         float *FY = FYbase + (t & 1) * 5 * TY * TX, *EX = EXbase + (t & 1) * 5 * TY, *EY = EYbase + (t & 1) * 5 * TX;
 
-        const T *sc = sbase(pc);
+        const T *sc = sbase(slot_c);
         float Gx[5], Gy[5];
         {   // x+ face of the own cell: cells i-2 .. i+3
             float tp[6][6];
@@ -367,7 +369,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         __syncthreads();                                   // the only barrier of the step
         if (tid == 0 && t + 9 < n_planes) {                      // slot of plane pc is free again
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            issue(t + 9);
+            issue(t + 9, slot_c);
         }
 
         // z+ face (cells k-2 .. k+3 of the own column), then the divergence
@@ -415,6 +417,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];
         }
         ax_c = ax_n; ay_c = ay_n; az_c = az_n;
+        slot_c = slot_c1;
+        if (++slot_n == NSLOT) { slot_n = 0; phase_n ^= 1; }
     }
 
     if (FUSE && a.wave) {
