@@ -126,14 +126,32 @@ def cpu_baseline(w, n_box=96, steps=2):
             % (wb.nx, wb.ny, wb.nz, w.name, steps), "ms_per_step": dt_wall / steps * 1e3}
 
 
-def alg_bytes(row, storage):
-    """Algorithmic HBM bytes per cell per launch: q and Sigma in the storage
-    type (s bytes), b and r in fp32.  source: 4 q reads + b write; jacobi (5 sweeps blocked, ideal):
-    rho + b + Sigma in + Sigma out; rhs: 5 q + Sigma reads + 5 r writes; rk_update: averaged over the
-    3 stages (q_n, q_s reads except stage 1, r read, q write)."""
+def alg_bytes(row, storage, fused=1):
+    """Algorithmic HBM bytes per cell per launch, averaged over the three stages:
+    q and Sigma in the storage type (s bytes), b and r in fp32.  source: 4 q reads + b write; jacobi
+    (5 sweeps blocked): rho + b + Sigma in + Sigma out; rhs: 5 q + Sigma reads, then either 5 r writes
+    (unfused) or the fused update: q_n reads in stages 2, 3 and 5 q writes; rk_update (unfused only)."""
     s = 4 if storage == "f32" else 2
-    return {"sigma_source": 4 * s + 4, "jacobi": 3 * s + 4, "rhs": 6 * s + 20,
+    rhs = 6 * s + (5 * s + 2 * 5 * s / 3.0 if fused else 20)
+    return {"sigma_source": 4 * s + 4, "jacobi": 3 * s + 4, "rhs": rhs,
             "rk_update": (5 * (s + 4 + s) + 2 * 5 * (2 * s + 4 + s)) / 3.0}[row]
+
+
+# Algorithmic fp32 operations per cell per launch (FMA = 2), counted on the oracle's formulas
+# (DESIGN.md section 5): rhs = 3 faces x (reconstruction 108 + two side fluxes 48 + LF 25 + lambda 2)
+# + cell wave speeds 15 + divergence 30 + RK stage 20; jacobi = 5 sweeps x 14 + coefficients 20;
+# source = 9 differences + velocities + traces.
+ALG_FLOP = {"sigma_source": 45.0, "jacobi": 90.0, "rhs": 614.0, "rk_update": 20.0}
+# DRAM bytes per cell per launch measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum,
+# profiles/r01_ncu_full_*): fp32 storage, stage-1 launch of the fused RHS kernel
+NCU_DRAM_BYTES_PER_CELL = {"f32": {"sigma_source": 20.8, "jacobi": 21.3, "rhs": 47.6}}
+
+
+def alu_peak_tflops():
+    """Plain FP32 ALU peak of a B200: 148 SMs x 128 lanes x 2 flop (FMA) x SM clock."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    mhz = float(json.load(open(p)).get("sm_max_mhz", 1965.0)) if os.path.exists(p) else 1965.0
+    return 148 * 128 * 2 * mhz * 1e6 / 1e12
 
 
 def reduce_max(value, world, device="cpu"):
@@ -212,16 +230,30 @@ def run_ours(args):
     step_ms_prof = sum(v[0] for v in rows.values()) / nprof
     dom = max(("sigma_source", "jacobi", "rhs", "rk_update"), key=lambda r: rows[r][0])
     peak, peak_src = measured_peaks()
-    ach = alg_bytes(dom, args.storage) * cells / (row_ms[dom] * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src, "alg_bytes_per_cell": alg_bytes(dom, args.storage),
-                "avg_launch_ms": row_ms[dom], "share_of_step": rows[dom][0] / nprof / step_ms_prof,
-                "rows_ms_per_call": row_ms,
-                "rows_frac_of_peak": {r: alg_bytes(r, args.storage) * cells / (row_ms[r] * 1e-3) / 1e9 / peak
-                                      for r in ("sigma_source", "jacobi", "rhs", "rk_update") if row_ms[r] > 0},
-                "step_hbm_frac_of_peak": (3 * (alg_bytes("sigma_source", args.storage) + alg_bytes("jacobi", args.storage)
-                                               + alg_bytes("rhs", args.storage) + alg_bytes("rk_update", args.storage))
-                                          * cells / (ms_step * 1e-3) / 1e9 / peak)}
+    main_rows = [r for r in ("sigma_source", "jacobi", "rhs", "rk_update") if row_ms[r] > 0]
+    hbm_gbs = {r: alg_bytes(r, args.storage, args.fused) * cells / (row_ms[r] * 1e-3) / 1e9 for r in main_rows}
+    alu_tf = {r: ALG_FLOP[r] * cells / (row_ms[r] * 1e-3) / 1e12 for r in main_rows}
+    alu_peak = alu_peak_tflops()
+    # the dominant kernel is reported against the roofline that binds it: the larger of the two fractions
+    if alu_tf[dom] / alu_peak > hbm_gbs[dom] / peak:
+        roofline = {"bound": "alu", "kernel": dom, "achieved": alu_tf[dom], "peak": alu_peak, "unit": "TFLOP/s",
+                    "frac": alu_tf[dom] / alu_peak,
+                    "peak_source": "148 SM x 128 fp32 lanes x 2 x sm_max_mhz (DESIGN.md section 5)",
+                    "alg_flop_per_cell": ALG_FLOP[dom]}
+    else:
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": hbm_gbs[dom], "peak": peak, "unit": "GB/s",
+                    "frac": hbm_gbs[dom] / peak, "peak_source": peak_src}
+    t_cell = NCU_DRAM_BYTES_PER_CELL.get(args.storage, {}).get(dom)
+    roofline.update({
+        "traffic": t_cell * cells if t_cell else None, "traffic_unit": "bytes per launch (ncu, see profiles/)",
+        "alg_bytes_per_cell": alg_bytes(dom, args.storage, args.fused),
+        "hbm": {"achieved_gbs": hbm_gbs[dom], "peak_gbs": peak, "frac": hbm_gbs[dom] / peak, "peak_source": peak_src},
+        "avg_launch_ms": row_ms[dom], "share_of_step": rows[dom][0] / nprof / step_ms_prof,
+        "rows_ms_per_call": row_ms,
+        "rows_hbm_frac": {r: hbm_gbs[r] / peak for r in main_rows},
+        "rows_alu_frac": {r: alu_tf[r] / alu_peak for r in main_rows},
+        "step_hbm_frac": sum(3 * alg_bytes(r, args.storage, args.fused) for r in main_rows) * cells
+        / (ms_step * 1e-3) / 1e9 / peak})
 
     # end to end through the C ABI with HOST buffers: set_state (H2D) + wave speed + step + get_state (D2H)
     e2e = None

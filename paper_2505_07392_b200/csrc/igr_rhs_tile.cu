@@ -17,6 +17,7 @@
 #include "igr_rhs_tile.cuh"
 
 #include <cstdio>
+#include <type_traits>
 #include <cstdlib>
 #include <cuda_fp16.h>
 #include <cuda_bf16.h>
@@ -90,7 +91,11 @@ struct Tile {
     static constexpr int FY_OFF = A_OFF + 2 * 2 * A_N * 4;           // float [2][5][TY][TX]
     static constexpr int EX_OFF = FY_OFF + 2 * 5 * TY * TX * 4;      // float [2][5][TY]
     static constexpr int EY_OFF = EX_OFF + 2 * 5 * TY * 4;           // float [2][5][TX]
-    static constexpr int BAR_OFF = (EY_OFF + 2 * 5 * TX * 4 + 7) / 8 * 8;
+    // reduced-precision storage: the current plane is converted ONCE to fp32 (two buffers by plane
+    // parity, same box layout, Sigma after the five q fields) so that the stencil taps need no cvt
+    static constexpr int CUR_N = (sizeof(T) == 2) ? 6 * PE : 0;      // floats per buffer
+    static constexpr int CUR_OFF = (EY_OFF + 2 * 5 * TX * 4 + 15) / 16 * 16;
+    static constexpr int BAR_OFF = (CUR_OFF + 2 * CUR_N * 4 + 7) / 8 * 8;
     static constexpr int TOTAL = BAR_OFF + NSLOT * 8;
 };
 
@@ -190,6 +195,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     float *FYbase = reinterpret_cast<float *>(smem + TL::FY_OFF);       // [2][5][TY][TX]
     float *EXbase = reinterpret_cast<float *>(smem + TL::EX_OFF);       // [2][5][TY]
     float *EYbase = reinterpret_cast<float *>(smem + TL::EY_OFF);       // [2][5][TX]
+    float *CUR = reinterpret_cast<float *>(smem + TL::CUR_OFF);         // [2][6][PE] (half storage only)
+    constexpr bool HALF = sizeof(T) == 2;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + TL::BAR_OFF);
 
     const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5, warp = ty;
@@ -269,6 +276,21 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             }
         }
     };
+    // half storage: plane p (ring slot `slot`) -> fp32 buffer of its parity, two elements per access
+    auto convert_plane = [&](int p, int slot) {
+        if (!HALF) return;
+        float2 *dq = reinterpret_cast<float2 *>(CUR + (p & 1) * TL::CUR_N);
+        const unsigned *sq = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT);
+        const unsigned *ss = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT + TL::QBYTES);
+        for (int e = tid; e < 3 * TL::PE; e += TX * TY) {                 // 6 PE elements = 3 PE pairs
+            const unsigned v = e < 5 * TL::PE / 2 ? sq[e] : ss[e - 5 * TL::PE / 2];
+            float2 o;
+            if (sizeof(T) == 2 && std::is_same<T, __half>::value) o = __half22float2(*reinterpret_cast<const __half2 *>(&v));
+            else o = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&v));
+            dq[e] = o;
+        }
+    };
+    convert_plane(3, 3);
     put_speeds(3, 3, ax_c, ay_c);                                  // plane of the first cell layer kz0
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
@@ -304,34 +326,38 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         float ax_n, ay_n, az_n;
         cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_n, ay_n, az_n);
         put_speeds(pc + 1, slot_c1, ax_n, ay_n);                  // read in the next step (after the barrier)
-        const T *qc = qbase(slot_c);
+        convert_plane(pc + 1, slot_c1);
+        // the current plane as seen by the stencil taps: the ring slot itself (fp32) or its fp32 copy
+        typedef typename std::conditional<HALF, float, T>::type TC;
+        const TC *qc = HALF ? reinterpret_cast<const TC *>(CUR + (pc & 1) * TL::CUR_N)
+                            : reinterpret_cast<const TC *>(qbase(slot_c));
         const float *A0 = Abase + (pc & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
         float *FY = FYbase + (t & 1) * 5 * TY * TX, *EX = EXbase + (t & 1) * 5 * TY, *EY = EYbase + (t & 1) * 5 * TX;
 
-        const T *sc = sbase(slot_c);
+        const TC *sc = HALF ? qc + 5 * TL::PE : reinterpret_cast<const TC *>(sbase(slot_c));
         float Gx[5], Gy[5];
         {   // x+ face of the own cell: cells i-2 .. i+3
             float tp[6][6];
-            const T *qb = qc + own;
+            const TC *qb = qc + own;
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
 #pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<T>(qb + f * TL::PE + (s - 2));
+                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2));
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<T>(sc + own + (s - 2));
+            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<TC>(sc + own + (s - 2));
             face_flux2<ORDER, 0>(tp, fmaxf(ax_c, A0[(ty + 1) * TL::AW + tx + 2]), gm1, Gx);
         }
         {   // y+ face: cells j-2 .. j+3
             float tp[6][6];
-            const T *qb = qc + own;
+            const TC *qb = qc + own;
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
 #pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<T>(qb + f * TL::PE + (s - 2) * TL::BX);
+                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<T>(sc + own + (s - 2) * TL::BX);
+            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<TC>(sc + own + (s - 2) * TL::BX);
             face_flux2<ORDER, 1>(tp, fmaxf(ay_c, A1[(ty + 2) * TL::AW + tx + 1]), gm1, Gy);
 #pragma unroll
             for (int c = 0; c < 5; ++c) FY[(c * TY + ty) * TX + tx] = Gy[c];
@@ -339,14 +365,14 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         if (warp == 2 % TY && tx < TY) {
             // faces on the tile's low-x edge: between box columns HX-1 | HX of row tx
             float tp[6][6], Ge[5];
-            const T *qb = qc + (3 + tx) * TL::BX + TL::HX - 1;
+            const TC *qb = qc + (3 + tx) * TL::BX + TL::HX - 1;
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
 #pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = lds<T>(qb + f * TL::PE + (s - 2));
+                for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2));
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = lds<T>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
+            for (int s = 0; s < 6; ++s) tp[5][s] = lds<TC>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
             face_flux2<ORDER, 0>(tp, fmaxf(A0[(tx + 1) * TL::AW + 0], A0[(tx + 1) * TL::AW + 1]), gm1, Ge);
 #pragma unroll
             for (int c = 0; c < 5; ++c) EX[c * TY + tx] = Ge[c];
@@ -354,14 +380,14 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         if (warp == 3 % TY) {
             // faces on the tile's low-y edge: between box rows 2 | 3 of column tx
             float tp[6][6], Ge[5];
-            const T *qb = qc + 2 * TL::BX + TL::HX + tx;
+            const TC *qb = qc + 2 * TL::BX + TL::HX + tx;
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
 #pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = lds<T>(qb + f * TL::PE + (s - 2) * TL::BX);
+                for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = lds<T>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
+            for (int s = 0; s < 6; ++s) tp[5][s] = lds<TC>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
             face_flux2<ORDER, 1>(tp, fmaxf(A1[0 * TL::AW + tx + 1], A1[1 * TL::AW + tx + 1]), gm1, Ge);
 #pragma unroll
             for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
