@@ -59,7 +59,7 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     // fp32 storage: incoming planes are staged by cp.async PF steps ahead (ring of PF + 1 stages of
     // rho, b, Sigma for the R*R columns); each thread reads back only what it copied itself
     float *STG = jb_smem + (2 + 2 * NS) * PP;                                           // [PF+1][3][R*R]
-    constexpr bool ASYNC = sizeof(T) == 4;
+    constexpr bool ASYNC = true;   // 2-byte storage: cp.async copies the aligned 4-byte word holding the element
 
     const int rx = threadIdx.x & 31, ry0 = threadIdx.x >> 5;
     const int gi = blockIdx.x * OT - NS + rx;
@@ -138,9 +138,10 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
         float *st = STG + stage * 3 * R * R + threadIdx.x;
 #pragma unroll
         for (int cc = 0; cc < CPT; ++cc) {
-            cp4(st + cc * NTHREADS, rho + (off_r[cc] + zr));
+            // (for 2-byte T the source address is rounded down to its 4-byte word)
+            cp4(st + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(rho + (off_r[cc] + zr)) & ~(uintptr_t)3));
             cp4(st + R * R + cc * NTHREADS, bsrc + (off_m[cc] + zm));
-            cp4(st + 2 * R * R + cc * NTHREADS, sin + (off_m[cc] + zm));
+            cp4(st + 2 * R * R + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(sin + (off_m[cc] + zm)) & ~(uintptr_t)3));
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -181,7 +182,16 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
                 const float *st = STG + (tau % (PF + 1)) * 3 * R * R + threadIdx.x;
 #pragma unroll
                 for (int cc = 0; cc < CPT; ++cc) {
-                    rho0[cc] = st[cc * NTHREADS]; b0[cc] = st[R * R + cc * NTHREADS]; s0[cc] = st[2 * R * R + cc * NTHREADS];
+                    b0[cc] = st[R * R + cc * NTHREADS];
+                    if (sizeof(T) == 4) {
+                        rho0[cc] = st[cc * NTHREADS]; s0[cc] = st[2 * R * R + cc * NTHREADS];
+                    } else {
+                        // pick the element out of its word: the parity of the element offset is the
+                        // same for every plane when the plane stride is even (it is: px is a multiple of 16)
+                        const T *wr = reinterpret_cast<const T *>(st + cc * NTHREADS);
+                        const T *ws = reinterpret_cast<const T *>(st + 2 * R * R + cc * NTHREADS);
+                        rho0[cc] = ldf(wr + (off_r[cc] & 1u)); s0[cc] = ldf(ws + (off_m[cc] & 1u));
+                    }
                 }
             } else {
 #pragma unroll

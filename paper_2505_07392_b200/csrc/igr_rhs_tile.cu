@@ -282,12 +282,20 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         float2 *dq = reinterpret_cast<float2 *>(CUR + (p & 1) * TL::CUR_N);
         const unsigned *sq = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT);
         const unsigned *ss = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT + TL::QBYTES);
-        for (int e = tid; e < 3 * TL::PE; e += TX * TY) {                 // 6 PE elements = 3 PE pairs
-            const unsigned v = e < 5 * TL::PE / 2 ? sq[e] : ss[e - 5 * TL::PE / 2];
-            float2 o;
-            if (sizeof(T) == 2 && std::is_same<T, __half>::value) o = __half22float2(*reinterpret_cast<const __half2 *>(&v));
-            else o = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&v));
-            dq[e] = o;
+        auto cv = [](unsigned v) {
+            if (std::is_same<T, __half>::value) return __half22float2(*reinterpret_cast<const __half2 *>(&v));
+            return __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&v));
+        };
+        constexpr int NT = TX * TY, NQ = 5 * TL::PE / 2, NSG = TL::PE / 2;       // pairs of q / of Sigma
+#pragma unroll
+        for (int it = 0; it < (NQ + NT - 1) / NT; ++it) {
+            const int e = tid + it * NT;
+            if ((it + 1) * NT <= NQ || e < NQ) dq[e] = cv(sq[e]);
+        }
+#pragma unroll
+        for (int it = 0; it < (NSG + NT - 1) / NT; ++it) {
+            const int e = tid + it * NT;
+            if ((it + 1) * NT <= NSG || e < NSG) dq[NQ + e] = cv(ss[e]);
         }
     };
     convert_plane(3, 3);
