@@ -202,6 +202,7 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
             const int slot1 = (u + NS - 1) % NS;                              // ring slot of plane p1
             const int ko = p0 - NS;                                           // output plane of this step
             const bool out_ok = ko >= kz0 && ko < kz0 + nkz;
+            float wz_old[CPT];
 #pragma unroll
             for (int cc = 0; cc < CPT; ++cc) {
                 RHO[par0][pos[cc]] = rho0[cc];
@@ -209,50 +210,76 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
 
                 // ---- coefficients of plane p1 (its densities were stored in the previous step);
                 // the slot held plane p1 - NS, whose W_z+ the last level still needs
-                const float wz_old = C[cc][slot1].wzp;
-                {
-                    const float *rp = &RHO[par1][pos[cc]];
-                    const float r1 = rho1[cc];
-                    Coef c;
-                    c.wxm = k22 * rcp_approx(r1 + rp[-1]);
-                    c.wxp = k22 * rcp_approx(r1 + rp[1]);
-                    c.wym = k22 * rcp_approx(r1 + rp[-P]);
-                    c.wyp = k22 * rcp_approx(r1 + rp[P]);
-                    c.wzp = k22 * rcp_approx(r1 + rho0[cc]);
-                    c.dinv = rcp_approx(rcp_approx(r1) + ((c.wxm + c.wxp) + (c.wym + c.wyp) + (wz_prev[cc] + c.wzp)));
-                    c.b = b1[cc];
-                    wz_prev[cc] = c.wzp;                                      // W_z- of the next plane
-                    C[cc][slot1] = c;
-                }
+                wz_old[cc] = C[cc][slot1].wzp;
+                const float *rp = &RHO[par1][pos[cc]];
+                const float r1 = rho1[cc];
+                Coef c;
+                c.wxm = k22 * rcp_approx(r1 + rp[-1]);
+                c.wxp = k22 * rcp_approx(r1 + rp[1]);
+                c.wym = k22 * rcp_approx(r1 + rp[-P]);
+                c.wyp = k22 * rcp_approx(r1 + rp[P]);
+                c.wzp = k22 * rcp_approx(r1 + rho0[cc]);
+                c.dinv = rcp_approx(rcp_approx(r1) + ((c.wxm + c.wxp) + (c.wym + c.wyp) + (wz_prev[cc] + c.wzp)));
+                c.b = b1[cc];
+                wz_prev[cc] = c.wzp;                                          // W_z- of the next plane
+                C[cc][slot1] = c;
+            }
 
-                // ---- levels: level l+1 advances plane c = p1 - l
-                float above = s0[cc];                                         // level-0 iterate at plane p0
+            // ---- levels: level l+1 advances plane c = p1 - l, both columns together.  The in-plane
+            // neighbours of level l+1's plane were written in the PREVIOUS step (other buffer of the
+            // pair), so they are fetched one level ahead of their use, before this level's stores.
+            float above[CPT], nb[CPT][4];
 #pragma unroll
-                for (int l = 0; l < NS; ++l) {
-                    const int c = p1 - l;
-                    const int slot = (u + 2 * NS - 1 - l) % NS;               // slot of plane c
-                    const int slot_m = (u + 2 * NS - 2 - l) % NS;             // slot of plane c - 1
+            for (int cc = 0; cc < CPT; ++cc) {
+                above[cc] = s0[cc];                                           // level-0 iterate at plane p0
+                const float *sp = &SP[0][par1][pos[cc]];
+                nb[cc][0] = sp[-1]; nb[cc][1] = sp[1]; nb[cc][2] = sp[-P]; nb[cc][3] = sp[P];
+            }
+#pragma unroll
+            for (int l = 0; l < NS; ++l) {
+                const int c = p1 - l;
+                const int slot = (u + 2 * NS - 1 - l) % NS;                   // slot of plane c
+                const int slot_m = (u + 2 * NS - 2 - l) % NS;                 // slot of plane c - 1
+                float nx[CPT][4];
+                if (l + 1 < NS) {
+#pragma unroll
+                    for (int cc = 0; cc < CPT; ++cc) {
+                        const float *sp = &SP[l + 1][(par1 + l + 1) & 1][pos[cc]];
+                        nx[cc][0] = sp[-1]; nx[cc][1] = sp[1]; nx[cc][2] = sp[-P]; nx[cc][3] = sp[P];
+                    }
+                }
+#pragma unroll
+                for (int cc = 0; cc < CPT; ++cc) {
                     const Coef &k = C[cc][slot];
-                    const float wzm = (l == NS - 1) ? wz_old : C[cc][slot_m].wzp;
-                    const float *sp = &SP[l][(par1 + l) & 1][pos[cc]];        // plane c of level l
+                    const float wzm = (l == NS - 1) ? wz_old[cc] : C[cc][slot_m].wzp;
                     const float ctr = centre[cc][l];
                     const float dn = (EDGE && !per_z && c == 0) ? ctr : below[cc][l];
-                    const float up = (EDGE && !per_z && c == g.nz - 1) ? ctr : above;
-                    float acc = k.b;
-                    acc = fmaf(k.wxm, sp[-1], acc);
-                    acc = fmaf(k.wxp, sp[1], acc);
-                    acc = fmaf(k.wym, sp[-P], acc);
-                    acc = fmaf(k.wyp, sp[P], acc);
-                    acc = fmaf(wzm, dn, acc);
-                    acc = fmaf(k.wzp, up, acc);
-                    const float fresh = acc * k.dinv;                         // level l+1 at plane c
+                    const float up = (EDGE && !per_z && c == g.nz - 1) ? ctr : above[cc];
+                    // two partial sums: shorter dependency chains
+                    float a0 = fmaf(k.wxm, nb[cc][0], k.b);
+                    float a1 = k.wxp * nb[cc][1];
+                    a0 = fmaf(k.wym, nb[cc][2], a0);
+                    a1 = fmaf(k.wyp, nb[cc][3], a1);
+                    a0 = fmaf(wzm, dn, a0);
+                    a1 = fmaf(k.wzp, up, a1);
+                    const float fresh = (a0 + a1) * k.dinv;                   // level l+1 at plane c
                     below[cc][l] = ctr;
-                    centre[cc][l] = above;
-                    above = fresh;
+                    centre[cc][l] = above[cc];
+                    above[cc] = fresh;
                     if (l + 1 < NS) put(SP[l + 1][(par1 + l) & 1], cc, fresh);
                 }
-                // `above` now holds the level-NS iterate at plane p1 - (NS - 1) = p0 - NS
-                if ((mask[cc] & ST_CORE) && out_ok) stf(sout + (off_o[cc] + usz * (unsigned)(ko + IGR_NG)), above);
+                if (l + 1 < NS) {
+#pragma unroll
+                    for (int cc = 0; cc < CPT; ++cc) {
+#pragma unroll
+                        for (int n = 0; n < 4; ++n) nb[cc][n] = nx[cc][n];
+                    }
+                }
+            }
+#pragma unroll
+            for (int cc = 0; cc < CPT; ++cc) {
+                // above[] now holds the level-NS iterate at plane p1 - (NS - 1) = p0 - NS
+                if ((mask[cc] & ST_CORE) && out_ok) stf(sout + (off_o[cc] + usz * (unsigned)(ko + IGR_NG)), above[cc]);
                 rho1[cc] = rho0[cc]; b1[cc] = b0[cc];
             }
             __syncthreads();
