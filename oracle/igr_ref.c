@@ -28,6 +28,8 @@ struct igr_ref_solver {
     double *u[3], *p, *c;    /* cell-centred primitives incl. ghosts                   */
     double *sig, *sig2, *b;  /* Sigma, Sigma ping-pong, source                         */
     double *flux[5];         /* numerical flux of one axis, stored at the left cell    */
+    double mu, zeta;         /* shear and bulk viscosity (0: inviscid Euler)           */
+    double *G[9];            /* cell-centred velocity gradient G[3a+b] = du_a/dx_b     */
 };
 
 static long IDX(const igr_ref_solver *s, int i, int j, int k)
@@ -114,6 +116,7 @@ int igr_ref_create(int nx, int ny, int nz, double dx, double gamma, double alpha
     s->p = alloc_field(s->np); s->c = alloc_field(s->np);
     s->sig = alloc_field(s->np); s->sig2 = alloc_field(s->np); s->b = alloc_field(s->np);
     for (int c = 0; c < 5; ++c) s->flux[c] = alloc_field(s->np);
+    for (int c = 0; c < 9; ++c) s->G[c] = NULL;
     *out = s;
     return 0;
 }
@@ -124,8 +127,19 @@ void igr_ref_destroy(igr_ref_solver *s)
     for (int c = 0; c < 5; ++c) { free(s->q[c]); free(s->qn[c]); free(s->r[c]); free(s->flux[c]); }
     for (int a = 0; a < 3; ++a) free(s->u[a]);
     free(s->p); free(s->c); free(s->sig); free(s->sig2); free(s->b);
+    for (int c = 0; c < 9; ++c) free(s->G[c]);
     for (int f = 0; f < 6; ++f) free(s->patches[f]);
     free(s);
+}
+
+/* NEXT-1: Newtonian viscous stress, eqs. (2), (3), (5). */
+int igr_ref_set_viscosity(igr_ref_solver *s, double mu, double zeta)
+{
+    if (!s || mu < 0 || zeta < 0) return -1;
+    s->mu = mu; s->zeta = zeta;
+    if ((mu > 0 || zeta > 0) && !s->G[0])
+        for (int c = 0; c < 9; ++c) s->G[c] = alloc_field(s->np);
+    return 0;
 }
 
 int igr_ref_set_storage(igr_ref_solver *s, int mode)
@@ -446,6 +460,52 @@ void igr_ref_lf_flux(int d, double gamma, const double *UL, const double *UR,
         F[c] = 0.5 * (FL[c] + FR[c]) - 0.5 * lambda * (UR[c] - UL[c]);
 }
 
+/* ---------------------------------------------------------------- viscous fluxes (NEXT-1)
+ * Second-order velocity gradients (L132), the same ones the Sigma source uses (L232), at the
+ * cell centres: G_ab = (u_a[i+e_b] - u_a[i-e_b]) / (2 dx) on the interior; ghosts of this derived
+ * field by the BC index map (wrap / clamp; reading A19).  They are reconstructed at the face with
+ * the reconstruction coefficients of the state (Alg. 1: vflux_L/R += coeff_L/R(q) du/dn),
+ * the face velocity comes from the reconstructed conservative state (L187-L189), and the two
+ * sides are averaged (reading A19: the paper only names `viscous(vflux_L, vflux_R, u_L, u_R)`):
+ *   tau_ab = mu (G_ab + G_ba) + (zeta - 2 mu / 3) delta_ab tr G                    (eq. 5)
+ *   F_visc along d = ( 0, -tau_xd, -tau_yd, -tau_zd, -(u . tau)_d )               (eqs. 2-3)   */
+static void velocity_gradients(igr_ref_solver *s)
+{
+    const long st[3] = { s->sx, s->sy, s->sz };
+    const double inv2dx = 1.0 / (2.0 * s->dx);
+    const int nx = s->nx, ny = s->ny, nz = s->nz;
+    #pragma omp parallel for
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                long id = IDX(s, i, j, k);
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        s->G[3 * a + b][id] = (s->u[a][id + st[b]] - s->u[a][id - st[b]]) * inv2dx;
+            }
+    #pragma omp parallel for
+    for (int k = -NG; k < nz + NG; ++k)
+        for (int j = -NG; j < ny + NG; ++j)
+            for (int i = -NG; i < nx + NG; ++i) {
+                if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) continue;
+                long src = IDX(s, map_index(i, nx, s->face[0]), map_index(j, ny, s->face[2]),
+                               map_index(k, nz, s->face[4]));
+                for (int c = 0; c < 9; ++c) s->G[c][IDX(s, i, j, k)] = s->G[c][src];
+            }
+}
+
+/* viscous flux along d from the face values of the gradient tensor and the velocity */
+void igr_ref_viscous_flux(int d, double mu, double zeta, const double *G9, const double *u3, double *F)
+{
+    double tr = G9[0] + G9[4] + G9[8];
+    double tau[3];                                   /* tau_ad, a = x, y, z */
+    for (int a = 0; a < 3; ++a)
+        tau[a] = mu * (G9[3 * a + d] + G9[3 * d + a]) + ((a == d) ? (zeta - 2.0 * mu / 3.0) * tr : 0.0);
+    F[0] = 0.0;
+    for (int a = 0; a < 3; ++a) F[1 + a] = -tau[a];
+    F[4] = -(u3[0] * tau[0] + u3[1] * tau[1] + u3[2] * tau[2]);
+}
+
 /* ---------------------------------------------------------------- steps 4-7: RHS
  * For each axis d (dimensional splitting, Alg. 1) and each face i+1/2 bounding an
  * interior cell: reconstruct the six fields (q and Sigma, Alg. 1 L183-L196, L205/L224),
@@ -457,6 +517,8 @@ int igr_ref_rhs(igr_ref_solver *s)
     const int n[3] = { s->nx, s->ny, s->nz };
     const long st[3] = { s->sx, s->sy, s->sz };
     for (int c = 0; c < 5; ++c) memset(s->r[c], 0, sizeof(double) * s->np);
+    const int viscous = (s->mu > 0 || s->zeta > 0);
+    if (viscous) velocity_gradients(s);
     for (int d = 0; d < 3; ++d) {
         /* faces: left cell index along d runs -1..n_d-1, other axes over the interior */
         int lo[3] = { 0, 0, 0 }, hi[3] = { n[0], n[1], n[2] };
@@ -479,6 +541,17 @@ int igr_ref_rhs(igr_ref_solver *s)
                     double lambda = lamL > lamR ? lamL : lamR;
                     double F[5];
                     igr_ref_lf_flux(d, s->gamma, UL, UR, sL, sR, lambda, F);
+                    if (viscous) {
+                        double GL[9], GR[9], Gf[9], uf[3], Fv[5];
+                        for (int c = 0; c < 9; ++c) {
+                            for (int t = -2; t <= 3; ++t) f6[t + 2] = s->G[c][id + t * st[d]];
+                            igr_ref_reconstruct(s->order, f6, &GL[c], &GR[c]);
+                            Gf[c] = 0.5 * (GL[c] + GR[c]);
+                        }
+                        for (int a = 0; a < 3; ++a) uf[a] = 0.5 * (UL[1 + a] / UL[0] + UR[1 + a] / UR[0]);
+                        igr_ref_viscous_flux(d, s->mu, s->zeta, Gf, uf, Fv);
+                        for (int c = 0; c < 5; ++c) F[c] += Fv[c];
+                    }
                     for (int c = 0; c < 5; ++c) s->flux[c][id] = F[c];
                 }
         #pragma omp parallel for

@@ -61,6 +61,8 @@ int  igr_ref_create(int nx, int ny, int nz, double dx, double gamma, double alph
                     int order, int n_jacobi, const igr_ref_bc *bc, igr_ref_solver **out);
 void igr_ref_destroy(igr_ref_solver *s);
 int  igr_ref_set_storage(igr_ref_solver *s, int mode);       /* IGR_REF_STORE_*         */
+/* NEXT-1: shear and bulk viscosity of eq. (5) (L64-L67); 0, 0 = inviscid Euler (default) */
+int  igr_ref_set_viscosity(igr_ref_solver *s, double mu, double zeta);
 
 /* interior-only host arrays, layout [5][nz][ny][nx] (state) or [nz][ny][nx] (scalar) */
 int  igr_ref_set_state(igr_ref_solver *s, const double *q);  /* also resets Sigma = 0   */
@@ -95,6 +97,8 @@ void igr_ref_reconstruct(int order, const double *f6, double *fL, double *fR);
 /* Sigma_L, Sigma_R and the wave speed lambda                                          */
 void igr_ref_lf_flux(int d, double gamma, const double *UL, const double *UR,
                      double sigL, double sigR, double lambda, double *F);
+/* viscous flux along d from face values of G[3a+b] = du_a/dx_b and of the velocity   */
+void igr_ref_viscous_flux(int d, double mu, double zeta, const double *G9, const double *u3, double *F);
 /* round x to the storage format (round to nearest even)                               */
 double igr_ref_round_storage(double x, int mode);
 

@@ -53,6 +53,9 @@ def lib():
         _lib.igr_ref_destroy.argtypes = [vp]
         _lib.igr_ref_destroy.restype = None
         _lib.igr_ref_set_storage.argtypes = [vp, C.c_int]
+        _lib.igr_ref_set_viscosity.argtypes = [vp, C.c_double, C.c_double]
+        _lib.igr_ref_viscous_flux.argtypes = [C.c_int, C.c_double, C.c_double, dp, dp, dp]
+        _lib.igr_ref_viscous_flux.restype = None
         for name in ("set_state", "get_state", "set_sigma", "get_sigma", "get_source", "get_rhs",
                      "set_source",
                      "max_wavespeed"):
@@ -119,6 +122,9 @@ class RefSolver:
 
     def set_storage(self, mode):
         assert lib().igr_ref_set_storage(self._h, mode) == 0
+
+    def set_viscosity(self, mu, zeta=0.0):
+        assert lib().igr_ref_set_viscosity(self._h, float(mu), float(zeta)) == 0
 
     def set_state(self, q):
         q = np.ascontiguousarray(q, dtype=np.float64)
@@ -207,6 +213,14 @@ def lf_flux(d, gamma, UL, UR, sigL, sigR, lam):
     UR = np.ascontiguousarray(UR, dtype=np.float64)
     F = np.empty(5)
     lib().igr_ref_lf_flux(d, gamma, _dptr(UL), _dptr(UR), sigL, sigR, lam, _dptr(F))
+    return F
+
+
+def viscous_flux(d, mu, zeta, G9, u3):
+    G9 = np.ascontiguousarray(G9, dtype=np.float64).reshape(9)
+    u3 = np.ascontiguousarray(u3, dtype=np.float64)
+    F = np.empty(5)
+    lib().igr_ref_viscous_flux(d, mu, zeta, _dptr(G9), _dptr(u3), _dptr(F))
     return F
 
 
