@@ -36,6 +36,8 @@ def parse():
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mu", type=float, default=0.0, help="shear viscosity (NEXT-1; 0 = Euler, the headline)")
+    ap.add_argument("--zeta", type=float, default=0.0, help="bulk viscosity")
     return ap.parse_args()
 
 
@@ -186,6 +188,8 @@ def run_ours(args):
     w = make_workload(args.workload)
     storage = {"f32": igr.STORE_F32, "f16": igr.STORE_F16, "bf16": igr.STORE_BF16}[args.storage]
     g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
+    if args.mu > 0 or args.zeta > 0:
+        g.set_viscosity(args.mu, args.zeta)          # unfused rows + viscous add-on kernel
     q0 = W.state(w, device=dev)
     g.set_state(q0)
     g.sync()
@@ -284,7 +288,7 @@ def run_ours(args):
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
-                      "storage": args.storage, "fused": args.fused, "n_jacobi": w.n_jacobi, "order": w.order,
+                      "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
                       "cfl": w.cfl, "parallelism": "replicas only" if world > 1 else "single GPU",
                       "l2": "inputs larger than L2 (no flush needed)" if cells * 4 > (126 << 20) else "inputs fit L2",
                       "wavespeed_query_every_step": True},

@@ -139,6 +139,13 @@ int igr_get_rhs(igr_solver *s, float *r);               /* r,   [5][nz][ny][nx] 
  * f: [nz+6][ny+6][nx+6] */
 int igr_get_padded(igr_solver *s, int c, float *f);
 
+/* ---- NEXT-1: Newtonian viscous stress of eqs. (2), (3), (5):
+ * tau_ab = mu (du_a/dx_b + du_b/dx_a) + (zeta - 2 mu/3) delta_ab div u, second-order velocity gradients
+ * (L132) reconstructed at the faces (Alg. 1), -tau and -u.tau added to the momentum and energy
+ * fluxes.  mu = zeta = 0 (default) is the inviscid path.  With viscosity on, igr_step runs the unfused
+ * rows (RHS, viscous add-on, update); nine fp32 gradient fields are allocated by this call. */
+int igr_set_viscosity(igr_solver *s, double mu, double zeta);
+
 /* ---- measurement hooks (bench.py).  Rows: 0 halo_bc, 1 sigma_source, 2 jacobi (sweeps + Sigma
  * ghosts), 3 rhs, 4 rk_update, 5 max_wavespeed (standalone reduction). */
 int igr_kernel_launches(igr_solver *s, long long *out);  /* kernels launched since igr_create     */

@@ -75,6 +75,8 @@ struct igr_solver {
     BcDesc bc;
     std::vector<void *> bc_allocs;   // device arrays of the inflow faces
     std::string err;
+    double mu = 0, zeta = 0;         // viscosity (NEXT-1); 0, 0: inviscid
+    float *grad[9] = {};             // velocity-gradient fields (allocated by igr_set_viscosity)
     long long launches = 0;          // kernels launched so far (igr_kernel_launches)
     bool profile = false;            // per-row CUDA-event timing (igr_profile)
     std::vector<cudaEvent_t> ev;     // start/stop pairs
@@ -306,6 +308,7 @@ void igr_destroy(igr_solver *s)
 {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
+    for (int c = 0; c < 9; ++c) if (s->grad[c]) cudaFree(s->grad[c]);
     for (void *p : s->bc_allocs) cudaFree(p);
     if (s->owns_base && s->base) cudaFree(s->base);
     delete s;
@@ -428,8 +431,9 @@ int igr_sigma_source(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     RowTimer t(s, 1, 1);
+    const bool viscous = s->mu > 0 || s->zeta > 0;
     launch_source(s->g, s->storage, s->st[s->cur], s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
-                  s->stream);
+                  viscous ? s->grad : nullptr, s->stream);
     return finish(s, "igr_sigma_source");
 }
 
@@ -475,6 +479,13 @@ int igr_rhs(igr_solver *s)
     } else {
         launch_rhs_simple(s->g, s->storage, s->st[s->cur], s->sig[s->sig_cur], s->r, p, s->stream);
     }
+    if (s->mu > 0 || s->zeta > 0) {
+        // viscous fluxes: ghosts of the gradient fields by the BC index map, then r += -div F_visc
+        for (int c = 0; c < 9; ++c) launch_halo_sigma(s->g, IGR_STORE_F32, s->grad[c], s->stream);
+        launch_viscous_add(s->g, s->storage, s->order, s->st[s->cur], s->grad, s->r, (float)s->mu, (float)s->zeta,
+                           p.inv_dx, s->stream);
+        s->launches += 10;
+    }
     return finish(s, "igr_rhs");
 }
 
@@ -511,7 +522,7 @@ int igr_step(igr_solver *s, double dt)
         if ((rc = igr_halo_bc(s)) != IGR_OK) return rc;
         if ((rc = igr_sigma_source(s)) != IGR_OK) return rc;
         if ((rc = igr_jacobi(s)) != IGR_OK) return rc;
-        if (s->fused && s->variant == IGR_VARIANT_TILED) {
+        if (s->fused && s->variant == IGR_VARIANT_TILED && !(s->mu > 0 || s->zeta > 0)) {
             // RHS + stage update + (stage 3) wave speed in one kernel: q^n = st[0] is only read
             // pointwise, the sub-steps alternate st[1], st[2]; stage 3 writes st[0] in place.
             RowTimer t(s, 3, 1);
@@ -556,6 +567,22 @@ int igr_max_wavespeed(igr_solver *s, double *out)
     *out = (double)v;
     if (h.nonfinite || !(v > 0.0f) || !std::isfinite(v))
         return s->fail(IGR_ERR_NONFINITE, "igr_max_wavespeed: non-finite state (NaN/Inf, or negative pressure/density)");
+    return IGR_OK;
+}
+
+int igr_set_viscosity(igr_solver *s, double mu, double zeta)
+{
+    if (!s || !(mu >= 0) || !(zeta >= 0)) return IGR_ERR_ARG;
+    if ((mu > 0 || zeta > 0) && !s->grad[0]) {
+        for (int c = 0; c < 9; ++c) {
+            if (cudaMalloc((void **)&s->grad[c], (size_t)s->g.np * 4) != cudaSuccess) {
+                cudaGetLastError();
+                return s->fail(IGR_ERR_ALLOC, "igr_set_viscosity: cudaMalloc of the gradient fields failed");
+            }
+            IGR_CUDA_OK(cudaMemsetAsync(s->grad[c], 0, (size_t)s->g.np * 4, s->stream));
+        }
+    }
+    s->mu = mu; s->zeta = zeta;
     return IGR_OK;
 }
 

@@ -25,7 +25,7 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_get_state", "igr_set_sigma", "igr_get_sigma", "igr_max_wavespeed", "igr_step",
            "igr_sync", "igr_last_error", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs",
            "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
-           "igr_kernel_launches", "igr_profile", "igr_profile_read"]
+           "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity"]
 
 
 class IgrError(RuntimeError):
@@ -79,6 +79,7 @@ def lib():
             getattr(L, n).argtypes = [vp]
         L.igr_kernel_launches.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.igr_profile.argtypes = [vp, C.c_int]
+        L.igr_set_viscosity.argtypes = [vp, C.c_double, C.c_double]
         L.igr_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.igr_last_error.argtypes = [vp]
         L.igr_last_error.restype = C.c_char_p
@@ -227,6 +228,9 @@ class Solver:
         self._check(lib().igr_rk_update(self._h, int(stage), float(dt)))
 
     ROWS = ("halo_bc", "sigma_source", "jacobi", "rhs", "rk_update", "max_wavespeed")
+
+    def set_viscosity(self, mu, zeta=0.0):
+        self._check(lib().igr_set_viscosity(self._h, float(mu), float(zeta)))
 
     def kernel_launches(self):
         v = C.c_longlong()
