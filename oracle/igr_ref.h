@@ -13,7 +13,8 @@
  * (P4), source on linear velocity fields (P5), Jacobi vs dense solve / contraction
  * 60/61 (P6), uniform state bitwise (P7), conservation (P8), scale covariance (P9),
  * entropy-wave convergence order (P10), Sod vs exact Riemann solution (P11), axis
- * permutation symmetry (P12), periodic-doubling and inflow mask (P13).
+ * permutation symmetry (P12), periodic-doubling and inflow mask (P13); viscous fluxes
+ * (NEXT-1): textbook stress cases, tau:grad u heating, discrete shear-wave decay (P14).
  * Parity unpinned by any external value (fixed by DESIGN.md readings A2-A5 only):
  * the 5-sweep truncation, the warm-start order, the choice of the LF wave speed and
  * the arithmetic-mean face density.
