@@ -20,7 +20,8 @@
 
 namespace {
 
-constexpr int R = 32;                       // region edge (threads per CTA = R*R)
+constexpr int R = 32;                       // region edge
+constexpr int cpt_small = 2;                // columns per thread for NS <= 3 (1 = 1024 threads: measured slower)
 
 struct Coef { float wxm, wxp, wym, wyp, wzp, dinv, b; };
 
@@ -39,18 +40,17 @@ __device__ __forceinline__ int rho_index(int i, int n, bool periodic)
     return min(max(i, -1), n);
 }
 
-constexpr int CPT = 2;                      // columns per thread: rows ry and ry + R/CPT of the region
-constexpr int PF = 3;                       // cp.async prefetch distance in planes (fp32 storage)
-constexpr int NTHREADS = R * R / CPT;       // 512 threads x <= 128 registers: the whole pipeline state
-                                            // (7 coefficients x NS planes + 2 NS iterate values per
-                                            // column) stays in registers without spilling
-
-template <typename T, int NS>
-__global__ void __launch_bounds__(NTHREADS, 1)
+constexpr int PF = 3;                       // cp.async prefetch distance in planes
+// CPT = columns per thread (rows ry and ry + R/CPT of the region).  NS = 4, 5: CPT = 2, 512 threads x
+// 128 registers hold the pipeline state (7 coefficients x NS planes + 2 NS iterate values per column);
+// CPT = 1 (1024 threads x 64 registers, no spills for NS <= 3) was measured slower and is not used.
+template <typename T, int NS, int CPT>
+__global__ void __launch_bounds__(R * R / CPT, 1)
 k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bsrc, const T *__restrict__ sin,
                  T *__restrict__ sout, float k2, int zc)
 {
     constexpr int OT = R - 2 * NS;
+    constexpr int NTHREADS = R * R / CPT;
     constexpr int P = R + 2;                 // padded plane pitch: a border of one cell, so that the
     constexpr int PP = P * (R + 2);          // four in-plane neighbours are at constant offsets
     extern __shared__ __align__(16) float jb_smem[];
@@ -317,14 +317,15 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
     const int smem = (2 + 2 * ns) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4;
 #define IGR_JB(NSV)                                                                                      \
     do {                                                                                                 \
+        constexpr int CPTV = (NSV <= 3) ? cpt_small : 2;                                                 \
         static bool configured = false;                                                                  \
         if (!configured) {                                                                               \
-            cudaFuncSetAttribute(k_jacobi_blocked<T, NSV>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+            cudaFuncSetAttribute(k_jacobi_blocked<T, NSV, CPTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                  (2 + 2 * NSV) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4);      \
             configured = true;                                                                           \
         }                                                                                                \
-        k_jacobi_blocked<T, NSV><<<grid, NTHREADS, smem, st>>>(g, (const T *)rho, b, (const T *)sin,        \
-                                                           (T *)sout, k2, zc);                           \
+        k_jacobi_blocked<T, NSV, CPTV><<<grid, R * R / CPTV, smem, st>>>(g, (const T *)rho, b, (const T *)sin, \
+                                                                    (T *)sout, k2, zc);                 \
     } while (0)
     switch (ns) {
     case 1: IGR_JB(1); break;

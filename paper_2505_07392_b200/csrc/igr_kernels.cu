@@ -205,7 +205,7 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
 // Streaming form: a CTA owns a 32 x 8 column of cells and marches along z.  Each cell's velocity is
 // computed once (one reciprocal per cell) and shared: in-plane neighbours through a triple-buffered
 // shared-memory plane with a one-cell halo, z neighbours in registers.  4 loads + 1 store per cell.
-constexpr int SRC_TX = 32, SRC_TY = 8, SRC_ZC = 64;
+constexpr int SRC_TX = 32, SRC_TY = 8, SRC_ZC = 128;
 
 struct GradPtrs { float *g[9]; };            // G[3a+b] = du_a/dx_b (viscous fluxes, NEXT-1); g[0] == NULL: off
 
