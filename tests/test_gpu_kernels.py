@@ -271,3 +271,41 @@ def test_conservation_to_roundoff_tiled_periodic():
         g.step(0.4 / shape[0] / g.max_wavespeed())
     tot = g.get_state().astype(np.float64).reshape(5, -1).sum(axis=1)
     assert np.all(np.abs(tot - tot0) <= 2e-7 * scale), (tot - tot0) / scale
+
+
+@pytest.mark.parametrize("shape", [(16, 8, 1), (1, 1, 1), (1, 7, 3), (33, 1, 2)])
+@pytest.mark.parametrize("bc", ["periodic", "extrap"])
+@pytest.mark.parametrize("mode", [dict(fused=1), dict(variant=igr.VARIANT_SIMPLE)], ids=["tiled_fused", "simple"])
+def test_degenerate_shapes_whole_step(shape, bc, mode):
+    """One-cell-thick and single-cell domains: every ghost is a wrap / clamp of the same few cells."""
+    g, r = make_pair(shape, bc, **mode)
+    q = smooth_state(*shape, seed=11)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    for _ in range(2):
+        dt = 0.3 / max(shape) / g.max_wavespeed()
+        g.step(dt); r.step(dt)
+    mx, l1 = parity.worst(g.get_state(), r.get_state())
+    assert mx <= 1e-5, (mx, l1)
+    assert parity.scalar_norms(g.get_sigma(), r.get_sigma(), floor=1e-6)[0] <= 1e-4
+
+
+@pytest.mark.parametrize("n_jacobi,alpha_factor", [(0, 10.0), (5, 0.0), (10, 10.0)])
+def test_degenerate_solver_parameters(n_jacobi, alpha_factor):
+    """No sweeps (Sigma stays at its warm start), alpha = 0 (Sigma = 0: plain Euler), ten sweeps (two
+    blocked passes)."""
+    nx, ny, nz = 37, 20, 13
+    dx = 1.0 / nx
+    g = igr.Solver(nx, ny, nz, dx, G, alpha_factor * dx * dx, n_jacobi=n_jacobi, fused=1)
+    r = R.RefSolver(nx, ny, nz, dx, G, alpha_factor * dx * dx, n_jacobi=n_jacobi)
+    q = smooth_state(nx, ny, nz, seed=12)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    for _ in range(2):
+        dt = 0.3 * dx / g.max_wavespeed()
+        g.step(dt); r.step(dt)
+    mx, l1 = parity.worst(g.get_state(), r.get_state())
+    assert mx <= 1e-5, (mx, l1)
+    sg, sr = g.get_sigma(), r.get_sigma()
+    if n_jacobi == 0 or alpha_factor == 0.0:
+        assert np.all(sg == 0.0) and np.all(sr == 0.0)
+    else:
+        assert parity.scalar_norms(sg, sr)[0] <= 1e-4
