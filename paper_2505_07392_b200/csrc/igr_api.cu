@@ -4,6 +4,7 @@
 #include "../../include/igr.h"
 #include "igr_kernels.h"
 #include "igr_rhs_tile.cuh"
+#include "igr_viscous.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -76,7 +77,8 @@ struct igr_solver {
     std::vector<void *> bc_allocs;   // device arrays of the inflow faces
     std::string err;
     double mu = 0, zeta = 0;         // viscosity (NEXT-1); 0, 0: inviscid
-    float *grad[9] = {};             // velocity-gradient fields (allocated by igr_set_viscosity)
+    float *tau = nullptr;            // six stress fields (allocated by igr_set_viscosity; igr_viscous.cuh)
+    ViscTileMaps vmaps;              // TMA maps of the tiled viscous kernel
     long long launches = 0;          // kernels launched so far (igr_kernel_launches)
     bool profile = false;            // per-row CUDA-event timing (igr_profile)
     std::vector<cudaEvent_t> ev;     // start/stop pairs
@@ -308,7 +310,7 @@ void igr_destroy(igr_solver *s)
 {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
-    for (int c = 0; c < 9; ++c) if (s->grad[c]) cudaFree(s->grad[c]);
+    if (s->tau) cudaFree(s->tau);
     for (void *p : s->bc_allocs) cudaFree(p);
     if (s->owns_base && s->base) cudaFree(s->base);
     delete s;
@@ -433,7 +435,7 @@ int igr_sigma_source(igr_solver *s)
     RowTimer t(s, 1, 1);
     const bool viscous = s->mu > 0 || s->zeta > 0;
     launch_source(s->g, s->storage, s->st[s->cur], s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
-                  viscous ? s->grad : nullptr, s->stream);
+                  viscous ? s->tau : nullptr, (float)s->mu, (float)s->zeta, s->stream);
     return finish(s, "igr_sigma_source");
 }
 
@@ -480,11 +482,17 @@ int igr_rhs(igr_solver *s)
         launch_rhs_simple(s->g, s->storage, s->st[s->cur], s->sig[s->sig_cur], s->r, p, s->stream);
     }
     if (s->mu > 0 || s->zeta > 0) {
-        // viscous fluxes: ghosts of the gradient fields by the BC index map, then r += -div F_visc
-        for (int c = 0; c < 9; ++c) launch_halo_sigma(s->g, IGR_STORE_F32, s->grad[c], s->stream);
-        launch_viscous_add(s->g, s->storage, s->order, s->st[s->cur], s->grad, s->r, (float)s->mu, (float)s->zeta,
-                           p.inv_dx, s->stream);
-        s->launches += 10;
+        // viscous fluxes: ghosts of the stress fields by the BC index map, then r += -div F_visc
+        launch_halo_fields(s->g, s->tau, 6, s->stream);
+        if (s->variant == IGR_VARIANT_TILED) {
+            ViscTileArgs a = {};
+            for (int c = 0; c < 5; ++c) { a.q[c] = s->st[s->cur].f[c]; a.r[c] = s->r[c]; }
+            a.tau = s->tau; a.inv_dx = p.inv_dx; a.zc = 0;
+            launch_viscous_tile(s->g, s->storage, s->order, false, s->vmaps.q[s->cur], s->vmaps.tau, a, s->stream);
+        } else {
+            launch_viscous_add(s->g, s->storage, s->order, s->st[s->cur], s->tau, s->r, p.inv_dx, s->stream);
+        }
+        s->launches += 2;
     }
     return finish(s, "igr_rhs");
 }
@@ -522,21 +530,35 @@ int igr_step(igr_solver *s, double dt)
         if ((rc = igr_halo_bc(s)) != IGR_OK) return rc;
         if ((rc = igr_sigma_source(s)) != IGR_OK) return rc;
         if ((rc = igr_jacobi(s)) != IGR_OK) return rc;
-        if (s->fused && s->variant == IGR_VARIANT_TILED && !(s->mu > 0 || s->zeta > 0)) {
+        const bool viscous = s->mu > 0 || s->zeta > 0;
+        if (s->fused && s->variant == IGR_VARIANT_TILED) {
             // RHS + stage update + (stage 3) wave speed in one kernel: q^n = st[0] is only read
             // pointwise, the sub-steps alternate st[1], st[2]; stage 3 writes st[0] in place.
-            RowTimer t(s, 3, 1);
-            RhsTileArgs a = {};
+            // With viscosity the inviscid RHS kernel stores r and the viscous kernel carries the update.
+            RowTimer t(s, 3, viscous ? 3 : 1);
             const int src = s->cur, dst = stage == 1 ? 1 : (stage == 2 ? 2 : 0);
-            for (int c = 0; c < 5; ++c) { a.qn[c] = s->st[0].f[c]; a.qout[c] = s->st[dst].f[c]; }
-            a.beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
-            a.dt = (float)dt; a.read_qn = stage != 1;
+            const float beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
+            if (stage == 3) IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
+            RhsTileArgs a = {};
             a.gamma = (float)s->gamma; a.inv_dx = (float)(1.0 / s->dx); a.zc = 0;
-            if (stage == 3) {
-                IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
-                a.wave = s->wave;
+            if (!viscous) {
+                for (int c = 0; c < 5; ++c) { a.qn[c] = s->st[0].f[c]; a.qout[c] = s->st[dst].f[c]; }
+                a.beta = beta; a.dt = (float)dt; a.read_qn = stage != 1;
+                if (stage == 3) a.wave = s->wave;
+                launch_rhs_tile(s->g, s->storage, s->order, true, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
+            } else {
+                for (int c = 0; c < 5; ++c) a.r[c] = s->r[c];
+                launch_rhs_tile(s->g, s->storage, s->order, false, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
+                launch_halo_fields(s->g, s->tau, 6, s->stream);
+                ViscTileArgs v = {};
+                for (int c = 0; c < 5; ++c) {
+                    v.q[c] = s->st[src].f[c]; v.r[c] = s->r[c]; v.qn[c] = s->st[0].f[c]; v.qout[c] = s->st[dst].f[c];
+                }
+                v.tau = s->tau; v.inv_dx = a.inv_dx; v.zc = 0;
+                v.beta = beta; v.dt = (float)dt; v.gamma = a.gamma; v.read_qn = stage != 1;
+                if (stage == 3) v.wave = s->wave;
+                launch_viscous_tile(s->g, s->storage, s->order, true, s->vmaps.q[src], s->vmaps.tau, v, s->stream);
             }
-            launch_rhs_tile(s->g, s->storage, s->order, true, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
             s->cur = dst;
             if (stage == 3) s->wave_valid = true;
             if ((rc = finish(s, "igr_step (fused rhs)")) != IGR_OK) return rc;
@@ -573,13 +595,17 @@ int igr_max_wavespeed(igr_solver *s, double *out)
 int igr_set_viscosity(igr_solver *s, double mu, double zeta)
 {
     if (!s || !(mu >= 0) || !(zeta >= 0)) return IGR_ERR_ARG;
-    if ((mu > 0 || zeta > 0) && !s->grad[0]) {
-        for (int c = 0; c < 9; ++c) {
-            if (cudaMalloc((void **)&s->grad[c], (size_t)s->g.np * 4) != cudaSuccess) {
-                cudaGetLastError();
-                return s->fail(IGR_ERR_ALLOC, "igr_set_viscosity: cudaMalloc of the gradient fields failed");
-            }
-            IGR_CUDA_OK(cudaMemsetAsync(s->grad[c], 0, (size_t)s->g.np * 4, s->stream));
+    if ((mu > 0 || zeta > 0) && !s->tau) {
+        if (cudaMalloc((void **)&s->tau, (size_t)s->g.np * 6 * 4) != cudaSuccess) {
+            cudaGetLastError();
+            s->tau = nullptr;
+            return s->fail(IGR_ERR_ALLOC, "igr_set_viscosity: cudaMalloc of the stress fields failed");
+        }
+        IGR_CUDA_OK(cudaMemsetAsync(s->tau, 0, (size_t)s->g.np * 6 * 4, s->stream));
+        if (s->variant == IGR_VARIANT_TILED) {
+            const char *msg = "";
+            if (visc_tile_make_maps(s->g, s->storage, s->st, 3, s->tau, &s->vmaps, &msg) != 0)
+                return s->fail(IGR_ERR_CUDA, msg);
         }
     }
     s->mu = mu; s->zeta = zeta;

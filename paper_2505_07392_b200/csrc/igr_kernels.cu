@@ -2,6 +2,7 @@
 // wave-speed reduction of libigr (sm_100a).  Citations are PAPER.md lines; readings are DESIGN.md's.
 // The tiled/TMA RHS kernel and the temporally blocked Jacobi kernel live in their own files.
 #include "igr_kernels.h"
+#include "igr_viscous.cuh"
 
 #define IGR_STORE_F32 0
 #define IGR_STORE_F16 1
@@ -186,6 +187,26 @@ __global__ void k_halo_sigma(Grid g, T *__restrict__ sig)
     }
 }
 
+// ghosts of `nf` derived fp32 fields (field stride g.np) by the index map alone: one launch
+__global__ void k_halo_fields(Grid g, float *__restrict__ base, int nf)
+{
+    const long long n = ghost_count(g);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        GhostCell c = decode_ghost(g, t);
+        const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
+                                    map_index(c.k, g.nz, g.bc[4]));
+        const long long dst = g.idx(c.i, c.j, c.k);
+        for (int f = 0; f < nf; ++f) base[f * g.np + dst] = base[f * g.np + src];
+    }
+}
+
+void launch_halo_fields(const Grid &g, float *base, int nf, cudaStream_t st)
+{
+    long long n = ghost_count(g);
+    k_halo_fields<<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, base, nf);
+}
+
 void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cudaStream_t st)
 {
     long long n = ghost_count(g);
@@ -207,11 +228,12 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
 // shared-memory plane with a one-cell halo, z neighbours in registers.  4 loads + 1 store per cell.
 constexpr int SRC_TX = 32, SRC_TY = 8, SRC_ZC = 128;
 
-struct GradPtrs { float *g[9]; };            // G[3a+b] = du_a/dx_b (viscous fluxes, NEXT-1); g[0] == NULL: off
-
+// GRAD: the same gradients also give the viscous stress tau (eq. 5; NEXT-1, igr_viscous.cuh), stored
+// as six fp32 fields; mu2 = 2 mu, lam2 = zeta - 2 mu / 3.
 template <typename T, bool GRAD>
 __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q, float *__restrict__ b,
-                                                            float alpha, float inv2dx, GradPtrs gp)
+                                                            float alpha, float inv2dx, TauPtrs tp, float mu,
+                                                            float lam2)
 {
     constexpr int PW = SRC_TX + 2, PH = SRC_TY + 2, PN = PW * PH;
     __shared__ float U[3][3][PN];                            // three plane buffers: one barrier per step
@@ -283,11 +305,13 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
             const unsigned id = col + usz * (unsigned)(k + IGR_NG);
             b[id] = alpha * (trsq + tr * tr);
             if (GRAD) {                       // the same second-order gradients feed the viscous stress (L232)
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-#pragma unroll
-                    for (int bb = 0; bb < 3; ++bb) gp.g[3 * a + bb][id] = G[a][bb];
-                }
+                const float lt = lam2 * tr, mu2 = 2.0f * mu;
+                tp.t[IGR_TAU_XX][id] = mu2 * G[0][0] + lt;
+                tp.t[IGR_TAU_XY][id] = mu * (G[0][1] + G[1][0]);
+                tp.t[IGR_TAU_XZ][id] = mu * (G[0][2] + G[2][0]);
+                tp.t[IGR_TAU_YY][id] = mu2 * G[1][1] + lt;
+                tp.t[IGR_TAU_YZ][id] = mu * (G[1][2] + G[2][1]);
+                tp.t[IGR_TAU_ZZ][id] = mu2 * G[2][2] + lt;
             }
         }
 #pragma unroll
@@ -296,14 +320,15 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
 }
 
 void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
-                   float *const grad[9], cudaStream_t st)
+                   float *tau, float mu, float zeta, cudaStream_t st)
 {
     dim3 grid((g.nx + SRC_TX - 1) / SRC_TX, (g.ny + SRC_TY - 1) / SRC_TY, (g.nz + SRC_ZC - 1) / SRC_ZC);
-    GradPtrs gp;
-    for (int c = 0; c < 9; ++c) gp.g[c] = grad ? grad[c] : nullptr;
+    TauPtrs tp;
+    for (int c = 0; c < 6; ++c) tp.t[c] = tau ? tau + (size_t)c * g.np : nullptr;
+    const float lam2 = zeta - 2.0f * mu / 3.0f;
     DISPATCH_STORAGE(storage, {
-        if (grad) k_source<T, true><<<grid, SRC_TX * SRC_TY, 0, st>>>(g, q, b, alpha, inv2dx, gp);
-        else k_source<T, false><<<grid, SRC_TX * SRC_TY, 0, st>>>(g, q, b, alpha, inv2dx, gp);
+        if (tau) k_source<T, true><<<grid, SRC_TX * SRC_TY, 0, st>>>(g, q, b, alpha, inv2dx, tp, mu, lam2);
+        else k_source<T, false><<<grid, SRC_TX * SRC_TY, 0, st>>>(g, q, b, alpha, inv2dx, tp, 0.f, 0.f);
     });
 }
 
@@ -557,75 +582,54 @@ void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, Wave
 }
 
 // ------------------------------------------------------------------------------ NEXT-1: viscous fluxes
-// Newtonian stress of eqs. (2), (3), (5).  The cell-centred second-order velocity
-// gradients G (written by k_source, ghosts by the BC index map) are reconstructed at the face with the
-// coefficients of the state (Alg. 1), the face velocity comes from the reconstructed
-// conservative state, the two sides are averaged (reading A19):
-//   tau_ad = mu (G_ad + G_da) + (zeta - 2 mu/3) delta_ad tr G,  F_visc = (0, -tau_xd, -tau_yd, -tau_zd, -u.tau_d)
-// First correct form: one thread per cell adds -div F_visc to r (both faces through one code
-// instance, so the two cells of a face see bitwise the same flux).
+// Simple form (igr_viscous.cuh has the formulas; igr_viscous_tile.cu the streaming form): one thread per
+// cell adds (H^+ - H^-)/dx of its six faces to r[1..4], both faces of a direction through one code
+// instance.
 template <typename T, int ORDER>
-__global__ void __launch_bounds__(128) k_viscous_add(Grid g, StagePtrs q, GradPtrs gp, float *r0, float *r1,
-                                                     float *r2, float *r3, float *r4, float mu, float zeta,
-                                                     float inv_dx)
+__global__ void __launch_bounds__(128) k_viscous_add(Grid g, StagePtrs q, const float *__restrict__ tau,
+                                                     float *r1, float *r2, float *r3, float *r4, float inv_dx)
 {
     const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
     if (i >= g.nx) return;
-    float *rr[5] = { r0, r1, r2, r3, r4 };
+    float *rr[4] = { r1, r2, r3, r4 };
     const long long st[3] = { 1, g.sy, g.sz };
     const long long id0 = g.idx(i, j, k);
-    const float lam2 = zeta - 2.0f * mu / 3.0f;
-    float acc[5] = { 0.f, 0.f, 0.f, 0.f, 0.f };
+    float acc[4] = { 0.f, 0.f, 0.f, 0.f };
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        float Fp[5], Fm[5];
+        float Hp[4], Hm[4];
 #pragma unroll 1
         for (int side = 0; side < 2; ++side) {
             const long long id = side ? id0 - st[d] : id0;          // left cell of the face
-            float f[6], l, r;
-            float Gf[9];
-#pragma unroll
-            for (int c = 0; c < 9; ++c) {
-#pragma unroll
-                for (int t = 0; t < 6; ++t) f[t] = gp.g[c][id + (t - 2) * st[d]];
-                reconstruct<ORDER>(f, l, r);
-                Gf[c] = 0.5f * (l + r);
-            }
-            float UL[4], UR[4];
+            float tq[4][6], tt[3][6], H[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
 #pragma unroll
-                for (int t = 0; t < 6; ++t) f[t] = ldf((const T *)q.f[c] + id + (t - 2) * st[d]);
-                reconstruct<ORDER>(f, UL[c], UR[c]);
+                for (int t = 0; t < 6; ++t) tq[c][t] = ldf((const T *)q.f[c] + id + (t - 2) * st[d]);
             }
-            const float il = 1.0f / UL[0], ir = 1.0f / UR[0];
-            const float uf[3] = { 0.5f * (UL[1] * il + UR[1] * ir), 0.5f * (UL[2] * il + UR[2] * ir),
-                                  0.5f * (UL[3] * il + UR[3] * ir) };
-            const float tr = Gf[0] + Gf[4] + Gf[8];
-            float tau[3];
 #pragma unroll
-            for (int a = 0; a < 3; ++a) tau[a] = mu * (Gf[3 * a + d] + Gf[3 * d + a]) + ((a == d) ? lam2 * tr : 0.f);
-            float F[5] = { 0.f, -tau[0], -tau[1], -tau[2], -(uf[0] * tau[0] + uf[1] * tau[1] + uf[2] * tau[2]) };
+            for (int a = 0; a < 3; ++a) {
+                const float *tf = tau + (long long)igr_visc::tau_field(d, a) * g.np;
 #pragma unroll
-            for (int c = 0; c < 5; ++c) { if (side) Fm[c] = F[c]; else Fp[c] = F[c]; }
+                for (int t = 0; t < 6; ++t) tt[a][t] = tf[id + (t - 2) * st[d]];
+            }
+            igr_visc::face<ORDER>(tq, tt, H);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { if (side) Hm[c] = H[c]; else Hp[c] = H[c]; }
         }
 #pragma unroll
-        for (int c = 1; c < 5; ++c) acc[c] -= (Fp[c] - Fm[c]) * inv_dx;
+        for (int c = 0; c < 4; ++c) acc[c] = __fadd_rn(acc[c], __fsub_rn(Hp[c], Hm[c]));
     }
 #pragma unroll
-    for (int c = 1; c < 5; ++c) rr[c][id0] += acc[c];
+    for (int c = 0; c < 4; ++c) rr[c][id0] = __fmaf_rn(inv_dx, acc[c], rr[c][id0]);
 }
 
-void launch_viscous_add(const Grid &g, int storage, int order, StagePtrs q, float *const grad[9],
-                        float *const r[5], float mu, float zeta, float inv_dx, cudaStream_t st)
+void launch_viscous_add(const Grid &g, int storage, int order, StagePtrs q, const float *tau,
+                        float *const r[5], float inv_dx, cudaStream_t st)
 {
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    GradPtrs gp;
-    for (int c = 0; c < 9; ++c) gp.g[c] = grad[c];
     DISPATCH_STORAGE(storage, {
-        if (order == 5)
-            k_viscous_add<T, 5><<<grid, 128, 0, st>>>(g, q, gp, r[0], r[1], r[2], r[3], r[4], mu, zeta, inv_dx);
-        else
-            k_viscous_add<T, 3><<<grid, 128, 0, st>>>(g, q, gp, r[0], r[1], r[2], r[3], r[4], mu, zeta, inv_dx);
+        if (order == 5) k_viscous_add<T, 5><<<grid, 128, 0, st>>>(g, q, tau, r[1], r[2], r[3], r[4], inv_dx);
+        else k_viscous_add<T, 3><<<grid, 128, 0, st>>>(g, q, tau, r[1], r[2], r[3], r[4], inv_dx);
     });
 }

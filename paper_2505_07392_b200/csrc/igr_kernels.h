@@ -26,12 +26,15 @@ void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cu
 void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st);
 
 // a2: b = alpha (tr((grad u)^2) + (tr grad u)^2)
-// `grad` (9 fp32 padded fields G[3a+b] = du_a/dx_b) is also written when not NULL (viscous fluxes)
+// `tau` (block of 6 fp32 padded fields, stride g.np: the viscous stress of eq. 5, igr_viscous.cuh) is
+// also written when not NULL
 void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
-                   float *const grad[9], cudaStream_t st);
-// NEXT-1: r += -div F_visc (eqs. 2, 3, 5); grad must have its ghosts filled (launch_halo_sigma, fp32)
-void launch_viscous_add(const Grid &g, int storage, int order, StagePtrs q, float *const grad[9],
-                        float *const r[5], float mu, float zeta, float inv_dx, cudaStream_t st);
+                   float *tau, float mu, float zeta, cudaStream_t st);
+// ghosts of nf derived fp32 fields (stride g.np) by the BC index map
+void launch_halo_fields(const Grid &g, float *base, int nf, cudaStream_t st);
+// NEXT-1, simple form: r[1..4] += -div F_visc (eqs. 2, 3, 5); tau must have its ghosts filled
+void launch_viscous_add(const Grid &g, int storage, int order, StagePtrs q, const float *tau,
+                        float *const r[5], float inv_dx, cudaStream_t st);
 
 // a3 (simple form): one Jacobi sweep, neighbours of Sigma through the BC index map
 void launch_jacobi_sweep(const Grid &g, int storage, const void *rho, const float *b,

@@ -92,3 +92,56 @@ def test_zero_viscosity_is_the_default_path_bitwise():
     for _ in range(2):
         g2.step(0.3 / shape[0] / g2.max_wavespeed())
     assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], g2.get_state())
+
+
+@pytest.mark.parametrize("bc", ["periodic", "mixed", "inflow_x"])
+@pytest.mark.parametrize("shape", [(37, 20, 13), (70, 33, 40)])
+def test_viscous_fused_update_equals_unfused_rows_bitwise(shape, bc):
+    """With viscosity the viscous kernel carries the stage update (rows a5/a6): same arithmetic as
+    igr_rhs + igr_rk_update, so the states agree bit for bit; both agree with the oracle."""
+    q = smooth_state(*shape, seed=8)
+    out, sig, wave = [], [], []
+    for fused in (0, 1):
+        g, r = pair(shape, bc, fused=fused)
+        g.set_state(q)
+        for _ in range(3):
+            v = g.max_wavespeed()
+            wave.append(v)
+            g.step(0.3 / shape[0] / v)
+        out.append(g.get_state()); sig.append(g.get_sigma())
+    assert np.array_equal(out[0], out[1]) and np.array_equal(sig[0], sig[1])
+    assert wave[:3] == wave[3:]
+    r.set_state(q.astype(np.float64))
+    for v in wave[:3]:
+        r.step(0.3 / shape[0] / v)
+    mx, l1 = parity.worst(out[1], r.get_state())
+    assert mx <= 1e-4, (mx, l1)
+
+
+@pytest.mark.parametrize("fmt", ["f16", "bf16"])
+@pytest.mark.parametrize("fused", [0, 1])
+def test_viscous_reduced_storage(fmt, fused):
+    """fp32 arithmetic on 2-byte state storage (C7) with the viscous rows: against the oracle with the same
+    storage emulation, criterion of tests/test_gpu_storage.py (most stored values identical, the rest a
+    few ulps of the storage format)."""
+    from test_gpu_storage import FMT, compare_stored
+    f = FMT[fmt]
+    shape = (40, 24, 19)
+    nx, ny, nz = shape
+    dx = 1.0 / nx
+    faces, patches = BCS["mixed"]
+    g = igr.Solver(nx, ny, nz, dx, G, 10 * dx * dx, faces=faces, patches=patches, storage=f["gpu"], fused=fused)
+    r = R.RefSolver(nx, ny, nz, dx, G, 10 * dx * dx, faces=faces, patches=patches, storage=f["ref"])
+    g.set_viscosity(MU, ZETA); r.set_viscosity(MU, ZETA)
+    q = smooth_state(*shape, seed=9)
+    g.set_state(q); r.set_state(q.astype(np.float64))
+    for _ in range(2):
+        dt = 0.3 * dx / g.max_wavespeed()
+        g.step(dt); r.step(dt)
+    a, b = g.get_state(), r.get_state()
+    for c in range(5):
+        same, within1, worst = compare_stored(a[c], b[c], f["pbits"])
+        # a flipped rounding of E (f16 ulp at 2.5: 2e-3) in a neighbouring cell moves a near-zero
+        # momentum by ~1e-5 one stage later: several ulps AT THE FLOOR magnitude, a small fraction of
+        # an ulp of the field's typical values -- hence 16 rather than the 8 of the three-step configs
+        assert same >= 0.97 and within1 >= 0.999 and worst <= 16, (c, same, within1, worst)
