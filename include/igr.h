@@ -142,8 +142,10 @@ int igr_get_padded(igr_solver *s, int c, float *f);
 /* ---- NEXT-1: Newtonian viscous stress of eqs. (2), (3), (5):
  * tau_ab = mu (du_a/dx_b + du_b/dx_a) + (zeta - 2 mu/3) delta_ab div u, second-order velocity gradients
  * (L132) reconstructed at the faces (Alg. 1), -tau and -u.tau added to the momentum and energy
- * fluxes.  mu = zeta = 0 (default) is the inviscid path.  With viscosity on, igr_step runs the unfused
- * rows (RHS, viscous add-on, update); nine fp32 gradient fields are allocated by this call. */
+ * fluxes.  mu = zeta = 0 (default) is the inviscid path.  With viscosity on, the source row also stores
+ * the six components of tau (six fp32 fields, allocated by this call with cudaMalloc: IGR_ERR_ALLOC if
+ * that fails), igr_rhs adds the viscous part to r, and igr_step (fused) lets the viscous kernel carry
+ * the stage update.  Both arguments must be >= 0 (IGR_ERR_ARG). */
 int igr_set_viscosity(igr_solver *s, double mu, double zeta);
 
 /* ---- measurement hooks (bench.py).  Rows: 0 halo_bc, 1 sigma_source, 2 jacobi (sweeps + Sigma
