@@ -92,7 +92,7 @@ int igr_ref_create(int nx, int ny, int nz, double dx, double gamma, double alpha
     for (int a = 0; a < 3; ++a) {   /* periodic must be on both faces of an axis */
         int lo = bc->face[2 * a], hi = bc->face[2 * a + 1];
         if ((lo == IGR_REF_BC_PERIODIC) != (hi == IGR_REF_BC_PERIODIC)) return -2;
-        if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return -2;
+        if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return -2;
     }
     igr_ref_solver *s = (igr_ref_solver *)calloc(1, sizeof(*s));
     if (!s) return -3;
@@ -231,6 +231,13 @@ int igr_ref_get_padded(const igr_ref_solver *s, int c, double *out)
     return 0;
 }
 
+int igr_ref_set_padded(igr_ref_solver *s, int c, const double *in)
+{
+    if (!s || !in || c < 0 || c > 5) return -1;
+    memcpy(c < 5 ? s->q[c] : s->sig, in, sizeof(double) * s->np);
+    return 0;
+}
+
 /* ---------------------------------------------------------------- boundary conditions
  * The paper gives no boundary conditions; BASELINE.json names periodic, extrapolation
  * outflow and fixed-state inflow patches.  SURVEY 8(c) "BC as an index map":
@@ -273,6 +280,19 @@ static const igr_ref_patch *find_patch(const igr_ref_solver *s, int face, int t0
     return best;
 }
 
+/* Domain decomposition (reading A20): a ghost cell that lies beyond an EXTERNAL face along any of its
+ * out-of-range axes belongs to the neighbouring sub-domain (or is an edge/corner cell no stencil reads):
+ * it is never written here. */
+static int ghost_is_external(const igr_ref_solver *s, int i, int j, int k)
+{
+    int idx[3] = { i, j, k }, n[3] = { s->nx, s->ny, s->nz };
+    for (int a = 0; a < 3; ++a) {
+        if (idx[a] < 0 && s->face[2 * a] == IGR_REF_BC_EXTERNAL) return 1;
+        if (idx[a] >= n[a] && s->face[2 * a + 1] == IGR_REF_BC_EXTERNAL) return 1;
+    }
+    return 0;
+}
+
 static const igr_ref_patch *inflow_patch_for_ghost(const igr_ref_solver *s, int i, int j, int k,
                                                    double *weight)
 {
@@ -301,6 +321,7 @@ int igr_ref_fill_ghosts(igr_ref_solver *s)
         for (int j = -NG; j < ny + NG; ++j)
             for (int i = -NG; i < nx + NG; ++i) {
                 if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) continue;
+                if (ghost_is_external(s, i, j, k)) continue;
                 long id = IDX(s, i, j, k);
                 double wgt;
                 const igr_ref_patch *pt = inflow_patch_for_ghost(s, i, j, k, &wgt);
@@ -338,6 +359,7 @@ int igr_ref_fill_sigma_ghosts(igr_ref_solver *s)
         for (int j = -NG; j < ny + NG; ++j)
             for (int i = -NG; i < nx + NG; ++i) {
                 if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) continue;
+                if (ghost_is_external(s, i, j, k)) continue;
                 long src = IDX(s, map_index(i, nx, s->face[0]), map_index(j, ny, s->face[2]),
                                map_index(k, nz, s->face[4]));
                 s->sig[IDX(s, i, j, k)] = s->sig[src];
@@ -488,6 +510,7 @@ static void velocity_gradients(igr_ref_solver *s)
         for (int j = -NG; j < ny + NG; ++j)
             for (int i = -NG; i < nx + NG; ++i) {
                 if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) continue;
+                if (ghost_is_external(s, i, j, k)) continue;
                 long src = IDX(s, map_index(i, nx, s->face[0]), map_index(j, ny, s->face[2]),
                                map_index(k, nz, s->face[4]));
                 for (int c = 0; c < 9; ++c) s->G[c][IDX(s, i, j, k)] = s->G[c][src];
@@ -605,13 +628,22 @@ static void rk_stage(igr_ref_solver *s, double a, double b, double dt)
 
 /* Sigma is a persistent field: each of the three solves is warm-started from the
  * previous one (L130, L138; reading A4); it is not RK-combined. */
+int igr_ref_stage(igr_ref_solver *s, int stage, double dt)
+{
+    if (!s || stage < 1 || stage > 3) return -1;
+    if (stage == 1)
+        for (int c = 0; c < 5; ++c) memcpy(s->qn[c], s->q[c], sizeof(double) * s->np);
+    igr_ref_eval_rhs(s);
+    if (stage == 1) rk_stage(s, 0.0, 1.0, dt);
+    else if (stage == 2) rk_stage(s, 0.75, 0.25, dt);
+    else rk_stage(s, 1.0 / 3.0, 2.0 / 3.0, dt);
+    return 0;
+}
+
 int igr_ref_step(igr_ref_solver *s, double dt)
 {
     if (!s) return -1;
-    for (int c = 0; c < 5; ++c) memcpy(s->qn[c], s->q[c], sizeof(double) * s->np);
-    igr_ref_eval_rhs(s); rk_stage(s, 0.0, 1.0, dt);
-    igr_ref_eval_rhs(s); rk_stage(s, 0.75, 0.25, dt);
-    igr_ref_eval_rhs(s); rk_stage(s, 1.0 / 3.0, 2.0 / 3.0, dt);
+    for (int stage = 1; stage <= 3; ++stage) igr_ref_stage(s, stage, dt);
     return 0;
 }
 

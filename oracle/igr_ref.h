@@ -35,6 +35,9 @@ extern "C" {
 #define IGR_REF_BC_PERIODIC 0
 #define IGR_REF_BC_EXTRAP   1
 #define IGR_REF_BC_INFLOW   2
+/* face shared with a neighbouring sub-domain (domain decomposition; DESIGN.md reading
+ * A20): ghosts beyond it are never filled by the oracle, the caller provides them (set_padded)    */
+#define IGR_REF_BC_EXTERNAL 3
 
 /* storage emulation ("FP32 compute, FP16 storage") */
 #define IGR_REF_STORE_F64  0
@@ -75,9 +78,11 @@ int  igr_ref_set_source(igr_ref_solver *s, const double *b); /* test hook for th
 int  igr_ref_get_rhs(const igr_ref_solver *s, double *r);    /* last computed r [5]...  */
 /* padded copy of q component c (0..4) or Sigma (c = 5): [nz+6][ny+6][nx+6]            */
 int  igr_ref_get_padded(const igr_ref_solver *s, int c, double *out);
+int  igr_ref_set_padded(igr_ref_solver *s, int c, const double *in);   /* inverse of get_padded */
 
 int  igr_ref_max_wavespeed(const igr_ref_solver *s, double *out);
 int  igr_ref_step(igr_ref_solver *s, double dt);             /* one SSP-RK3 step        */
+int  igr_ref_stage(igr_ref_solver *s, int stage, double dt); /* stage 1, 2, 3 of that step */
 
 /* the pieces of one RHS evaluation L(q, Sigma_prev) -> (r, Sigma), in order           */
 int  igr_ref_fill_ghosts(igr_ref_solver *s);   /* step 1: ghosts of q + primitives      */

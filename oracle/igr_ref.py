@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "igr_ref.c")
 _LIB = os.path.join(_HERE, "libigr_ref.so")
 
-PERIODIC, EXTRAP, INFLOW = 0, 1, 2
+PERIODIC, EXTRAP, INFLOW, EXTERNAL = 0, 1, 2, 3
 STORE_F64, STORE_F32, STORE_F16, STORE_BF16 = 0, 1, 2, 3
 
 
@@ -61,7 +61,9 @@ def lib():
                      "max_wavespeed"):
             getattr(_lib, "igr_ref_" + name).argtypes = [vp, dp]
         _lib.igr_ref_get_padded.argtypes = [vp, C.c_int, dp]
+        _lib.igr_ref_set_padded.argtypes = [vp, C.c_int, dp]
         _lib.igr_ref_step.argtypes = [vp, C.c_double]
+        _lib.igr_ref_stage.argtypes = [vp, C.c_int, C.c_double]
         for name in ("fill_ghosts", "source", "jacobi_sweep", "solve_sigma", "fill_sigma_ghosts",
                      "rhs", "eval_rhs"):
             getattr(_lib, "igr_ref_" + name).argtypes = [vp]
@@ -168,8 +170,16 @@ class RefSolver:
         assert lib().igr_ref_max_wavespeed(self._h, C.byref(v)) == 0
         return v.value
 
+    def set_padded(self, c, a):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        assert a.shape == (self.nz + 6, self.ny + 6, self.nx + 6)
+        assert lib().igr_ref_set_padded(self._h, c, _dptr(a)) == 0
+
     def step(self, dt):
         assert lib().igr_ref_step(self._h, float(dt)) == 0
+
+    def stage(self, stage, dt):
+        assert lib().igr_ref_stage(self._h, int(stage), float(dt)) == 0
 
     def fill_ghosts(self):
         lib().igr_ref_fill_ghosts(self._h)
