@@ -48,6 +48,9 @@ typedef enum {
 #define IGR_BC_PERIODIC 0    /* wrap modulo n; must be set on both faces of the axis               */
 #define IGR_BC_EXTRAP   1    /* zeroth-order extrapolation (clamp to the nearest interior cell)    */
 #define IGR_BC_INFLOW   2    /* fixed-state circular patches, extrapolation outside them           */
+#define IGR_BC_EXTERNAL 3    /* face shared with a neighbouring sub-domain (DESIGN.md */
+                             /* reading A20): ghosts beyond it are never written by the solver, the  */
+                             /* caller fills them (igr_pull_halo); sweeps clamp at it                */
 
 /* storage precision of q and Sigma in device memory; arithmetic is always fp32 */
 #define IGR_STORE_F32  0
@@ -147,6 +150,46 @@ int igr_get_padded(igr_solver *s, int c, float *f);
  * that fails), igr_rhs adds the viscous part to r, and igr_step (fused) lets the viscous kernel carry
  * the stage update.  Both arguments must be >= 0 (IGR_ERR_ARG). */
 int igr_set_viscosity(igr_solver *s, double mu, double zeta);
+
+/* ---- NEXT-2: z-slab domain decomposition, one halo exchange per RK stage (the
+ * paper scales by rectilinear decomposition with GPU-direct neighbour exchange, PAPER.md L258, L297-L311;
+ * DESIGN.md section 9, reading A20).  A rank's solver works on its owned planes extended by 8 overlap
+ * planes towards every neighbour; those z faces are IGR_BC_EXTERNAL.  One stage on the extended slab is
+ * exact on the owned planes (5 sweeps + 3 stencil planes = 8); after every stage the overlap and ghost
+ * planes (11 per side, q and Sigma) are overwritten with the neighbour's owned planes.  z is the slowest
+ * axis: a plane range of one field is ONE contiguous chunk, moved by cudaMemcpyAsync device-to-device
+ * (the copy engines over NVLink when the neighbour is another GPU whose allocation was opened with
+ * igr_ipc_open).  Ordering across ranks is the caller's (a barrier after the stage and after the pull:
+ * paper_2505_07392_b200/dist.py); the plan comes from paper_2505_07392_b200/slab.py. */
+typedef struct {
+    unsigned char ipc_handle[64]; /* cudaIpcMemHandle_t of the allocation (valid iff owns_memory)          */
+    uint64_t base;                /* address of that allocation in the OWNING process                      */
+    uint64_t q_offset[3][5];      /* bytes from base: state buffer b, field c (padded arrays)              */
+    uint64_t sig_offset[2];       /* bytes from base: the two Sigma buffers                                */
+    uint64_t plane_bytes;         /* one padded z-plane of one field                                       */
+    int32_t nz, storage;          /* local interior planes; IGR_STORE_*                                    */
+    int32_t cur, sig_cur;         /* buffers holding the current state / Sigma at the time of the call     */
+    int32_t owns_memory;          /* 1: the library allocated (cudaMalloc) -> the handle can be opened     */
+    int32_t reserved;
+} igr_export;
+
+/* one stage (1, 2, 3 in that order) of igr_step: halo, source, sweeps, RHS, update */
+int igr_stage(igr_solver *s, int stage, double dt);
+int igr_export_fields(igr_solver *s, igr_export *out);
+/* open / close a neighbour's allocation in this process (other process, same node).  *peer_base is the
+ * address HERE of peer->base THERE.  IGR_ERR_CUDA if the driver refuses (no peer access, same process). */
+int igr_ipc_open(const igr_export *peer, void **peer_base);
+int igr_ipc_close(void *peer_base);
+/* register (peer != NULL) or drop (peer == NULL) the neighbour on side 0 (z-) / 1 (z+): my planes
+ * [dst_plane, dst_plane + count) take its planes [src_plane, src_plane + count), interior-relative
+ * indices (my ghost planes are -3..-1 and nz..nz+2; the source must be interior planes of the peer).
+ * peer_base: its allocation as addressable here (igr_ipc_open, or peer->base inside one process).
+ * IGR_ERR_BC if that face is not IGR_BC_EXTERNAL, IGR_ERR_ARG on a shape / range mismatch. */
+int igr_set_neighbor(igr_solver *s, int side, const igr_export *peer, const void *peer_base,
+                     int dst_plane, int src_plane, int count);
+/* enqueue the copies of q (5 fields of the current buffer) and Sigma from every registered neighbour
+ * on the solver's stream; invalidates the cached wave speed */
+int igr_pull_halo(igr_solver *s);
 
 /* ---- measurement hooks (bench.py).  Rows: 0 halo_bc, 1 sigma_source, 2 jacobi (sweeps + Sigma
  * ghosts), 3 rhs, 4 rk_update, 5 max_wavespeed (standalone reduction). */

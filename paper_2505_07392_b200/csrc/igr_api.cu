@@ -79,6 +79,12 @@ struct igr_solver {
     double mu = 0, zeta = 0;         // viscosity (NEXT-1); 0, 0: inviscid
     float *tau = nullptr;            // six stress fields (allocated by igr_set_viscosity; igr_viscous.cuh)
     ViscTileMaps vmaps;              // TMA maps of the tiled viscous kernel
+    struct Neighbor {                // NEXT-2: neighbouring slab on z- / z+ (igr_set_neighbor)
+        bool active = false;
+        igr_export desc;
+        const char *base = nullptr;  // the neighbour's allocation as addressable from this process
+        int dst = 0, src = 0, count = 0;
+    } nb[2];
     long long launches = 0;          // kernels launched so far (igr_kernel_launches)
     bool profile = false;            // per-row CUDA-event timing (igr_profile)
     std::vector<cudaEvent_t> ev;     // start/stop pairs
@@ -93,6 +99,8 @@ struct igr_solver {
         return code;
     }
 };
+
+static_assert(IGR_BC_EXTERNAL == kBcExternal, "igr.h and igr_common.cuh disagree");
 
 namespace {
 
@@ -250,8 +258,9 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     if (storage < 0 || storage > 2) return IGR_ERR_ARG;
     for (int a = 0; a < 3; ++a) {
         const int lo = bc->face[2 * a], hi = bc->face[2 * a + 1];
-        if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return IGR_ERR_BC;
+        if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return IGR_ERR_BC;
         if ((lo == IGR_BC_PERIODIC) != (hi == IGR_BC_PERIODIC)) return IGR_ERR_BC;
+        if (a < 2 && (lo == IGR_BC_EXTERNAL || hi == IGR_BC_EXTERNAL)) return IGR_ERR_BC;   // z slabs only
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return IGR_ERR_CUDA; }
@@ -521,11 +530,15 @@ int igr_rk_update(igr_solver *s, int stage, double dt)
     return finish(s, "igr_rk_update");
 }
 
-int igr_step(igr_solver *s, double dt)
+int igr_stage(igr_solver *s, int stage, double dt)
 {
-    if (!s) return IGR_ERR_ARG;
-    if (s->cur != 0) return s->fail(IGR_ERR_ARG, "igr_step: called in the middle of a step");
-    for (int stage = 1; stage <= 3; ++stage) {
+    if (!s || stage < 1 || stage > 3) return IGR_ERR_ARG;
+    {
+        const int fused3 = (s->fused && s->variant == IGR_VARIANT_TILED) ? 2 : 1;
+        const int want = stage == 1 ? 0 : (stage == 2 ? 1 : fused3);
+        if (s->cur != want) return s->fail(IGR_ERR_ARG, "igr_stage: stages must run in the order 1, 2, 3");
+    }
+    {
         int rc;
         if ((rc = igr_halo_bc(s)) != IGR_OK) return rc;
         if ((rc = igr_sigma_source(s)) != IGR_OK) return rc;
@@ -567,6 +580,97 @@ int igr_step(igr_solver *s, double dt)
             if ((rc = igr_rk_update(s, stage, dt)) != IGR_OK) return rc;
         }
     }
+    return IGR_OK;
+}
+
+int igr_step(igr_solver *s, double dt)
+{
+    if (!s) return IGR_ERR_ARG;
+    if (s->cur != 0) return s->fail(IGR_ERR_ARG, "igr_step: called in the middle of a step");
+    for (int stage = 1; stage <= 3; ++stage) {
+        const int rc = igr_stage(s, stage, dt);
+        if (rc != IGR_OK) return rc;
+    }
+    return IGR_OK;
+}
+
+// ------------------------------------------------------------------------- NEXT-2: slab exchange
+// z is the slowest axis of the padded layout: a range of planes of one field is one contiguous chunk.
+int igr_export_fields(igr_solver *s, igr_export *out)
+{
+    if (!s || !out) return IGR_ERR_ARG;
+    memset(out, 0, sizeof *out);
+    out->base = (uint64_t)(uintptr_t)s->base;
+    for (int b = 0; b < 3; ++b)
+        for (int c = 0; c < 5; ++c) out->q_offset[b][c] = (uint64_t)((char *)s->st[b].f[c] - s->base);
+    for (int b = 0; b < 2; ++b) out->sig_offset[b] = (uint64_t)((char *)s->sig[b] - s->base);
+    out->plane_bytes = (uint64_t)s->g.sz * (s->storage == IGR_STORE_F32 ? 4 : 2);
+    out->nz = s->g.nz; out->storage = s->storage;
+    out->cur = s->cur; out->sig_cur = s->sig_cur;
+    out->owns_memory = s->owns_base ? 1 : 0;
+    if (s->owns_base) {
+        cudaIpcMemHandle_t h;
+        static_assert(sizeof h == sizeof out->ipc_handle, "igr_export.ipc_handle must hold a cudaIpcMemHandle_t");
+        IGR_CUDA_OK(cudaIpcGetMemHandle(&h, s->base));
+        memcpy(out->ipc_handle, &h, sizeof h);
+    }
+    return IGR_OK;
+}
+
+int igr_ipc_open(const igr_export *peer, void **peer_base)
+{
+    if (!peer || !peer_base || !peer->owns_memory) return IGR_ERR_ARG;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, peer->ipc_handle, sizeof h);
+    *peer_base = nullptr;
+    if (cudaIpcOpenMemHandle(peer_base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        cudaGetLastError();
+        return IGR_ERR_CUDA;
+    }
+    return IGR_OK;
+}
+
+int igr_ipc_close(void *peer_base)
+{
+    if (!peer_base) return IGR_ERR_ARG;
+    if (cudaIpcCloseMemHandle(peer_base) != cudaSuccess) { cudaGetLastError(); return IGR_ERR_CUDA; }
+    return IGR_OK;
+}
+
+int igr_set_neighbor(igr_solver *s, int side, const igr_export *peer, const void *peer_base, int dst_plane,
+                     int src_plane, int count)
+{
+    if (!s || side < 0 || side > 1) return IGR_ERR_ARG;
+    igr_solver::Neighbor &nb = s->nb[side];
+    if (!peer) { nb.active = false; return IGR_OK; }            // unregister
+    if (!peer_base || count < 1) return IGR_ERR_ARG;
+    if (s->g.bc[4 + side] != kBcExternal)
+        return s->fail(IGR_ERR_BC, "igr_set_neighbor: that z face is not IGR_BC_EXTERNAL");
+    const uint64_t pb = (uint64_t)s->g.sz * (s->storage == IGR_STORE_F32 ? 4 : 2);
+    if (peer->plane_bytes != pb || peer->storage != s->storage)
+        return s->fail(IGR_ERR_ARG, "igr_set_neighbor: the neighbour's planes have another shape or element type");
+    if (dst_plane < -IGR_NG || dst_plane + count > s->g.nz + IGR_NG || src_plane < 0 || src_plane + count > peer->nz)
+        return s->fail(IGR_ERR_ARG, "igr_set_neighbor: plane range outside the padded array / the neighbour's interior");
+    nb.active = true; nb.desc = *peer; nb.base = (const char *)peer_base;
+    nb.dst = dst_plane; nb.src = src_plane; nb.count = count;
+    return IGR_OK;
+}
+
+int igr_pull_halo(igr_solver *s)
+{
+    if (!s) return IGR_ERR_ARG;
+    const size_t pb = (size_t)s->g.sz * (s->storage == IGR_STORE_F32 ? 4 : 2);
+    for (int side = 0; side < 2; ++side) {
+        const igr_solver::Neighbor &nb = s->nb[side];
+        if (!nb.active) continue;
+        const size_t doff = (size_t)(nb.dst + IGR_NG) * pb, soff = (size_t)(nb.src + IGR_NG) * pb, n = (size_t)nb.count * pb;
+        for (int c = 0; c < 5; ++c)
+            IGR_CUDA_OK(cudaMemcpyAsync((char *)s->st[s->cur].f[c] + doff, nb.base + nb.desc.q_offset[s->cur][c] + soff, n,
+                                        cudaMemcpyDeviceToDevice, s->stream));
+        IGR_CUDA_OK(cudaMemcpyAsync((char *)s->sig[s->sig_cur] + doff, nb.base + nb.desc.sig_offset[s->sig_cur] + soff, n,
+                                    cudaMemcpyDeviceToDevice, s->stream));
+    }
+    s->wave_valid = false;          // the overlap planes changed: the cached wave speed is stale
     return IGR_OK;
 }
 

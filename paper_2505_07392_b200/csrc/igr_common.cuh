@@ -34,6 +34,17 @@ __host__ __device__ inline int map_index(int i, int n, int bc_lo)
     return i < 0 ? 0 : n - 1;
 }
 
+// Domain decomposition (igr.h IGR_BC_EXTERNAL; reading A20): a ghost cell beyond an external face
+// along any of its out-of-range axes is the neighbouring sub-domain's (or an edge/corner cell no stencil
+// reads): the halo kernels never write it.  Everywhere else an external face acts like a clamp.
+constexpr int kBcExternal = 3;
+__host__ __device__ inline bool ghost_is_external(const Grid &g, int i, int j, int k)
+{
+    return (i < 0 && g.bc[0] == kBcExternal) || (i >= g.nx && g.bc[1] == kBcExternal) ||
+           (j < 0 && g.bc[2] == kBcExternal) || (j >= g.ny && g.bc[3] == kBcExternal) ||
+           (k < 0 && g.bc[4] == kBcExternal) || (k >= g.nz && g.bc[5] == kBcExternal);
+}
+
 // ---- storage <-> fp32 (FP16 storage, FP32 compute)
 __device__ __forceinline__ float ldf(const float *p) { return *p; }
 __device__ __forceinline__ float ldf(const __half *p) { return __half2float(*p); }

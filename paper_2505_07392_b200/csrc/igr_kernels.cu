@@ -144,6 +144,7 @@ __global__ void k_halo_q(Grid g, StagePtrs q, BcDesc bc)
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
          t += (long long)gridDim.x * blockDim.x) {
         GhostCell c = decode_ghost(g, t);
+        if (ghost_is_external(g, c.i, c.j, c.k)) continue;
         const long long dst = g.idx(c.i, c.j, c.k);
         const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
                                     map_index(c.k, g.nz, g.bc[4]));
@@ -181,6 +182,7 @@ __global__ void k_halo_sigma(Grid g, T *__restrict__ sig)
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
          t += (long long)gridDim.x * blockDim.x) {
         GhostCell c = decode_ghost(g, t);
+        if (ghost_is_external(g, c.i, c.j, c.k)) continue;
         const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
                                     map_index(c.k, g.nz, g.bc[4]));
         sig[g.idx(c.i, c.j, c.k)] = sig[src];
@@ -194,6 +196,7 @@ __global__ void k_halo_fields(Grid g, float *__restrict__ base, int nf)
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
          t += (long long)gridDim.x * blockDim.x) {
         GhostCell c = decode_ghost(g, t);
+        if (ghost_is_external(g, c.i, c.j, c.k)) continue;
         const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
                                     map_index(c.k, g.nz, g.bc[4]));
         const long long dst = g.idx(c.i, c.j, c.k);

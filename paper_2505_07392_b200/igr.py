@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libigr.so")
 
 OK, ERR_ARG, ERR_BC, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
-BC_PERIODIC, BC_EXTRAP, BC_INFLOW = 0, 1, 2
+BC_PERIODIC, BC_EXTRAP, BC_INFLOW, BC_EXTERNAL = 0, 1, 2, 3
 STORE_F32, STORE_F16, STORE_BF16 = 0, 1, 2
 VARIANT_TILED, VARIANT_SIMPLE = 0, 1
 _STATUS = {0: "IGR_OK", -1: "IGR_ERR_ARG", -2: "IGR_ERR_BC", -3: "IGR_ERR_ALLOC", -4: "IGR_ERR_CUDA",
@@ -25,7 +25,8 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_get_state", "igr_set_sigma", "igr_get_sigma", "igr_max_wavespeed", "igr_step",
            "igr_sync", "igr_last_error", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs",
            "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
-           "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity"]
+           "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity", "igr_stage",
+           "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo"]
 
 
 class IgrError(RuntimeError):
@@ -47,6 +48,14 @@ class Options(C.Structure):
     _fields_ = [("storage", C.c_int32), ("fused", C.c_int32), ("variant", C.c_int32),
                 ("reserved", C.c_int32), ("stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class Export(C.Structure):
+    """igr_export (include/igr.h): plain bytes, can be shipped to another rank as they are."""
+    _fields_ = [("ipc_handle", C.c_ubyte * 64), ("base", C.c_uint64), ("q_offset", (C.c_uint64 * 5) * 3),
+                ("sig_offset", C.c_uint64 * 2), ("plane_bytes", C.c_uint64), ("nz", C.c_int32),
+                ("storage", C.c_int32), ("cur", C.c_int32), ("sig_cur", C.c_int32),
+                ("owns_memory", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -81,6 +90,12 @@ def lib():
         L.igr_profile.argtypes = [vp, C.c_int]
         L.igr_set_viscosity.argtypes = [vp, C.c_double, C.c_double]
         L.igr_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.igr_stage.argtypes = [vp, C.c_int, C.c_double]
+        L.igr_export_fields.argtypes = [vp, C.POINTER(Export)]
+        L.igr_ipc_open.argtypes = [C.POINTER(Export), C.POINTER(vp)]
+        L.igr_ipc_close.argtypes = [vp]
+        L.igr_set_neighbor.argtypes = [vp, C.c_int, C.POINTER(Export), vp, C.c_int, C.c_int, C.c_int]
+        L.igr_pull_halo.argtypes = [vp]
         L.igr_last_error.argtypes = [vp]
         L.igr_last_error.restype = C.c_char_p
         _lib = L
@@ -112,6 +127,21 @@ def _addr(a, shape, writable=False):
     if writable:
         assert a.flags.writeable
     return a.ctypes.data
+
+
+def ipc_open(peer):
+    """Address in this process of another process's allocation described by `peer` (an Export)."""
+    base = C.c_void_p()
+    rc = lib().igr_ipc_open(C.byref(peer), C.byref(base))
+    if rc != OK:
+        raise IgrError(rc, "igr_ipc_open")
+    return base.value
+
+
+def ipc_close(base):
+    rc = lib().igr_ipc_close(C.c_void_p(base))
+    if rc != OK:
+        raise IgrError(rc, "igr_ipc_close")
 
 
 class Solver:
@@ -226,6 +256,26 @@ class Solver:
 
     def rk_update(self, stage, dt):
         self._check(lib().igr_rk_update(self._h, int(stage), float(dt)))
+
+    # ---- NEXT-2: slab exchange (include/igr.h)
+    def stage(self, stage, dt):
+        self._check(lib().igr_stage(self._h, int(stage), float(dt)))
+
+    def export_fields(self):
+        e = Export()
+        self._check(lib().igr_export_fields(self._h, C.byref(e)))
+        return e
+
+    def set_neighbor(self, side, peer, peer_base, dst_plane, src_plane, count):
+        """peer: Export of the neighbour (None: drop it); peer_base: its allocation as addressable here."""
+        if peer is None:
+            self._check(lib().igr_set_neighbor(self._h, int(side), None, None, 0, 0, 0))
+        else:
+            self._check(lib().igr_set_neighbor(self._h, int(side), C.byref(peer), C.c_void_p(peer_base),
+                                               int(dst_plane), int(src_plane), int(count)))
+
+    def pull_halo(self):
+        self._check(lib().igr_pull_halo(self._h))
 
     ROWS = ("halo_bc", "sigma_source", "jacobi", "rhs", "rk_update", "max_wavespeed")
 

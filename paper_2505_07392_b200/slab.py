@@ -132,11 +132,13 @@ def receives(slab, peer_slab_of):
 
 def sends(slab, peer_slab_of):
     """The transfers of my neighbours that read from me (for two-sided exchanges): Transfer.peer is the
-    receiver, src are MY planes, dst THEIR planes."""
+    receiver, side the RECEIVER's side, src are MY planes, dst THEIR planes."""
     out = []
+    n = slab.halo
     for nb in sorted({r for r in (slab.lo, slab.hi) if r >= 0}):
         p = peer_slab_of(nb)
-        for t in receives(p, lambda r: slab if r == slab.rank else peer_slab_of(r)):
-            if t.peer == slab.rank:
-                out.append(Transfer(nb, t.side, t.dst, t.src, t.count))
+        if p.lo == slab.rank:                          # I am below them: they take my last n owned planes
+            out.append(Transfer(nb, 0, -NG, slab.own_hi - n, n))
+        if p.hi == slab.rank:                          # I am above them: they take my first n owned planes
+            out.append(Transfer(nb, 1, p.own_hi, slab.own_lo, n))
     return out

@@ -1,0 +1,173 @@
+"""NEXT-2 on the GPU: z-slab decomposition with the pull exchange of the
+C library (igr_set_neighbor / igr_pull_halo).  On the owned planes the slabs reproduce the single-domain
+CUDA run BITWISE, and the single-domain run is the one the other GPU tests hold against the oracle.
+
+One GPU is enough for correctness: (a) all slabs in one process, the "neighbour allocation" is another
+solver's memory on the same device; (b) two PROCESSES on cuda:0 with a gloo rendezvous, the neighbour's
+allocation opened through CUDA IPC exactly as on two GPUs (no kernel ever waits on another process: the
+ordering is host barriers)."""
+import dataclasses
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2505_07392_b200 import dist as D
+from paper_2505_07392_b200 import igr, slab as S
+from paper_2505_07392_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def jets_tall():
+    w = W.jets9(n=64, radius=4, pitch=14)
+    return dataclasses.replace(w, ny=40, nz=96)
+
+
+def tg_periodic():
+    return dataclasses.replace(W.taylor_green(32), nz=72)
+
+
+def run_global(w, n_steps, visc=None, **kw):
+    g = igr.Solver.for_workload(w, **kw)
+    if visc:
+        g.set_viscosity(*visc)
+    g.set_state(W.state(w).numpy())
+    dts = []
+    for _ in range(n_steps):
+        dt = w.cfl * w.dx / g.max_wavespeed()
+        dts.append(dt)
+        g.step(dt)
+    return g.get_state(), g.get_sigma(), dts, g.max_wavespeed()
+
+
+@pytest.mark.parametrize("mode", [dict(fused=1), dict(fused=0), dict(variant=igr.VARIANT_SIMPLE),
+                                  dict(fused=1, storage=igr.STORE_F16)],
+                         ids=["tiled_fused", "tiled", "simple", "f16_fused"])
+@pytest.mark.parametrize("case,nranks", [("jets", 2), ("jets", 3), ("tg", 2), ("tg", 4)])
+def test_local_slabs_equal_the_global_run_bitwise(case, nranks, mode):
+    w = jets_tall() if case == "jets" else tg_periodic()
+    q, sig, dts, vend = run_global(w, 3, **mode)
+    slabs = D.make_local(w, nranks, **mode)
+    for dt in dts:
+        v = max(s.solver.max_wavespeed() for s in slabs)
+        assert w.cfl * w.dx / v == dt                      # the global maximum is the maximum over the slabs
+        D.step_local(slabs, dt)
+    assert max(s.solver.max_wavespeed() for s in slabs) == vend
+    for s in slabs:
+        sl = s.slab
+        assert np.array_equal(s.owned_state(), q[:, sl.z0:sl.z1])
+        assert np.array_equal(s.owned_sigma(), sig[sl.z0:sl.z1])
+        idx = np.arange(sl.e0, sl.e1) % w.nz                # overlap planes: just refreshed by the pull
+        assert np.array_equal(s.solver.get_state(), q[:, idx])
+    for s in slabs:
+        s.close()
+
+
+def test_local_slabs_with_viscosity():
+    w = tg_periodic()
+    q, sig, dts, _ = run_global(w, 2, visc=(0.02, 0.01), fused=1)
+    slabs = D.make_local(w, 2, fused=1)
+    for s in slabs:
+        s.solver.set_viscosity(0.02, 0.01)
+    for dt in dts:
+        D.step_local(slabs, dt)
+    for s in slabs:
+        assert np.array_equal(s.owned_state(), q[:, s.slab.z0:s.slab.z1])
+        s.close()
+
+
+def test_seven_overlap_planes_are_not_enough_on_the_gpu(monkeypatch):
+    """The CUDA sweeps clamp at the extended boundary in every sweep: 5 contaminated planes + 3 stencil
+    planes.  With 7 overlap planes the owned plane next to the cut differs from the global run."""
+    w = tg_periodic()
+    q, _, dts, _ = run_global(w, 2, fused=1)
+    monkeypatch.setattr(S, "OVERLAP", 7)
+    orig = S.make_slab
+    monkeypatch.setattr(S, "make_slab", lambda w_, r, n, overlap=7: orig(w_, r, n, overlap=7))
+    slabs = D.make_local(w, 2, fused=1)
+    for dt in dts:
+        D.step_local(slabs, dt)
+    s = slabs[0]
+    assert not np.array_equal(s.owned_state(), q[:, s.slab.z0:s.slab.z1])
+    for s in slabs:
+        s.close()
+
+
+def test_exchange_abi_errors():
+    w = tg_periodic()
+    g = igr.Solver.for_workload(w)                          # periodic in z: no external face
+    e = g.export_fields()
+    assert e.nz == w.nz and e.owns_memory == 0 and e.plane_bytes > 0
+    with pytest.raises(igr.IgrError) as ei:
+        g.set_neighbor(0, e, e.base, -3, 0, 11)
+    assert ei.value.code == igr.ERR_BC
+    sl = D.SlabSolver(w, rank=0, nranks=2, exchange="local")
+    e2 = sl.solver.export_fields()
+    assert e2.owns_memory == 1
+    with pytest.raises(igr.IgrError) as ei:                 # source planes must be interior planes of the peer
+        sl.solver.set_neighbor(0, e2, e2.base, -3, e2.nz - 5, 11)
+    assert ei.value.code == igr.ERR_ARG
+    with pytest.raises(igr.IgrError) as ei:                 # stages in order
+        sl.solver.stage(2, 1e-3)
+    assert ei.value.code == igr.ERR_ARG
+    with pytest.raises(igr.IgrError):                       # external faces are z faces only
+        igr.Solver(8, 8, 8, 0.1, 1.4, 0.1, faces=(3, 1, 0, 0, 0, 0))
+    sl.close()
+
+
+# ------------------------------------------------------------------ two processes, one GPU, CUDA IPC
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, exchange, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        w = jets_tall()
+        s = D.SlabSolver(w, exchange=exchange, fused=1)
+        s.set_initial_state()
+        dts = []
+        for _ in range(3):
+            dt = w.cfl * w.dx / s.max_wavespeed()
+            dts.append(dt)
+            s.step(dt)
+        vend = s.max_wavespeed()
+        g = igr.Solver.for_workload(w, fused=1)
+        g.set_state(W.state(w).numpy())
+        for dt in dts:
+            assert w.cfl * w.dx / g.max_wavespeed() == dt
+            g.step(dt)
+        ok = np.array_equal(s.owned_state(), g.get_state()[:, s.slab.z0:s.slab.z1]) and \
+            np.array_equal(s.owned_sigma(), g.get_sigma()[s.slab.z0:s.slab.z1]) and vend == g.max_wavespeed()
+        dist.barrier()
+        s.close()
+        out.put((rank, bool(ok)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("exchange", ["ipc", "sendrecv"])
+def test_two_processes_on_one_gpu(exchange):
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, exchange, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=600) for _ in range(world))
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert res == [(0, True), (1, True)]
