@@ -7,8 +7,10 @@
 A "step" is one pass of the whole hot path (halo/BC, source, Jacobi, RHS, RK update, x3 stages) over
 the synthetic many-jet workload (config 5 of BASELINE.json at N=1).  Prints ONE JSON line.
 metric = grind time ns/(cell*eqn*RHS) = t_step / (cells * 5 * 3); lower is better.
-Multi-GPU: the path's halo exchange is not built yet, so --gpus N runs N independent
-replicas ("replicas only"): value = time / (total cells * 15), max over ranks.
+Multi-GPU (--gpus N under torchrun, one rank per GPU): weak scaling by z slabs: the
+job is the workload stacked N times along z, every rank owns one copy's planes plus 8 overlap planes per
+neighbour and pulls its halo planes from the neighbours after every RK stage (CUDA IPC peer copies, or
+torch.distributed send/recv); value = time / (total OWNED cells * 15), time = max over ranks.
 """
 import argparse
 import json
@@ -36,6 +38,13 @@ def parse():
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--exchange", default="ipc", choices=["ipc", "sendrecv"],
+                    help="N > 1: halo planes by CUDA IPC peer copies (falls back to sendrecv if IPC is refused) "
+                         "or by torch.distributed send/recv")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="N > 1: rendezvous backend")
+    ap.add_argument("--one-gpu", action="store_true",
+                    help="N > 1: every rank on cuda:0 (functional check of the exchange path on a 1-GPU box; "
+                         "use with --backend gloo; the timing is meaningless)")
     ap.add_argument("--mu", type=float, default=0.0, help="shear viscosity (NEXT-1; 0 = Euler, the headline)")
     ap.add_argument("--zeta", type=float, default=0.0, help="bulk viscosity")
     return ap.parse_args()
@@ -168,7 +177,7 @@ def reduce_max(value, world, device="cpu"):
 
 
 def job_numbers(ms_step, cells_per_rank, world):
-    """Whole-job metric of `world` replicas that each advance `cells_per_rank` cells in ms_step (max
+    """Whole-job metric of `world` ranks that each advance `cells_per_rank` owned cells in ms_step (max
     over ranks): grind time per (cell*eqn*RHS) of the job and aggregate cell updates per second."""
     total = cells_per_rank * world
     return {"grind_ns": ms_step * 1e6 / (total * 15), "cell_updates_per_s": total / (ms_step * 1e-3)}
@@ -181,19 +190,42 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.one_gpu:
+        local = 0
     torch.cuda.set_device(local)
     dev = "cuda:%d" % local
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device(dev))
+        else:
+            dist.init_process_group("gloo")
+    rdev = dev if args.backend == "nccl" else "cpu"      # where the scalar reductions live
     w = make_workload(args.workload)
     storage = {"f32": igr.STORE_F32, "f16": igr.STORE_F16, "bf16": igr.STORE_BF16}[args.storage]
-    g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
+    cells = w.n_cells                     # cells OWNED per rank (weak scaling: the job has world x cells)
+    ss = None
+    if world > 1:
+        # z-slab decomposition: the job is the workload stacked `world` times along z,
+        # every rank owns w.nz planes and computes 8 overlap planes per neighbour on top of them
+        import dataclasses
+        from paper_2505_07392_b200 import dist as D, slab as S
+        wg = dataclasses.replace(w, name="%s_x%dz" % (w.name, world), nz=w.nz * world)
+        ss = D.SlabSolver(wg, exchange=args.exchange, device=dev, storage=storage, fused=args.fused)
+        g = ss.solver
+        q0 = S.local_state(wg, ss.slab, device=dev)
+    else:
+        g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
+        q0 = W.state(w, device=dev)
     if args.mu > 0 or args.zeta > 0:
-        g.set_viscosity(args.mu, args.zeta)          # unfused rows + viscous add-on kernel
-    q0 = W.state(w, device=dev)
-    g.set_state(q0)
+        g.set_viscosity(args.mu, args.zeta)
+
+    def load_initial():
+        g.set_state(q0)
+        if ss:
+            ss.exchange()                 # ghost planes from the neighbours
+
+    load_initial()
     g.sync()
-    cells = w.n_cells
 
     def barrier():
         if world > 1:
@@ -201,20 +233,22 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     resets = [0]
+    solver = ss if ss else g              # max_wavespeed (max over ranks) and step (+ exchange per stage)
 
     def one_step():
         # The purely linear scheme eventually loses positivity on the under-resolved jets (F1:
-        # config 5 after ~137 steps).  The library reports it (IGR_ERR_NONFINITE); a long benchmark then
-        # restarts from the device-resident initial state and says so in the JSON line ("resets").
+        # config 5 after ~137 steps).  The library reports it (IGR_ERR_NONFINITE, on every rank after the
+        # max-reduction); a long benchmark then restarts from the device-resident initial state and says so
+        # in the JSON line ("resets").
         try:
-            lam = g.max_wavespeed()
+            lam = solver.max_wavespeed()
         except igr.IgrError as e:
             if e.code != igr.ERR_NONFINITE:
                 raise
-            g.set_state(q0)
+            load_initial()
             resets[0] += 1
-            lam = g.max_wavespeed()
-        g.step(w.cfl * w.dx / lam)
+            lam = solver.max_wavespeed()
+        solver.step(w.cfl * w.dx / lam)
 
     for _ in range(max(args.warmup, 3)):
         one_step()
@@ -231,7 +265,7 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = g.kernel_launches() - l0
     clocks = sampler.stop()
-    ms = reduce_max(ms, world, dev)
+    ms = reduce_max(ms, world, rdev)
     ms_step = ms / args.steps
     job = job_numbers(ms_step, cells, world)
     grind = job["grind_ns"]
@@ -239,8 +273,20 @@ def run_ours(args):
     # per-row CUDA-event timing on the solver's stream (separate region, same state)
     nprof = max(1, min(args.steps, 5))
     g.profile(True)
+    t_ex = [0.0]
+    if ss:                                # host time of the exchanges (syncs, barriers, peer copies)
+        inner = ss.exchange
+
+        def timed_exchange():
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            inner()
+            t_ex[0] += time.perf_counter() - t0
+        ss.exchange = timed_exchange
     for _ in range(nprof):
         one_step()
+    if ss:
+        ss.exchange = inner
     rows = g.profile_read()
     g.profile(False)
     row_ms = {r: (v[0] / v[1] if v[1] else 0.0) for r, v in rows.items()}
@@ -275,24 +321,27 @@ def run_ours(args):
     # end to end through the C ABI with HOST buffers: set_state (H2D) + wave speed + step + get_state (D2H)
     e2e = None
     if args.e2e_steps > 0:
+        lw = ss.slab.local if ss else w      # the arrays the rank's C-ABI calls move (extended slab)
         try:
-            host = torch.empty((5, w.nz, w.ny, w.nx), dtype=torch.float32, pin_memory=True)
+            host = torch.empty((5, lw.nz, lw.ny, lw.nx), dtype=torch.float32, pin_memory=True)
             pinned = True
         except RuntimeError:
-            host = torch.empty((5, w.nz, w.ny, w.nx), dtype=torch.float32)
+            host = torch.empty((5, lw.nz, lw.ny, lw.nx), dtype=torch.float32)
             pinned = False
-        g.set_state(q0)                          # a fresh state: the e2e steps never meet a reset
+        load_initial()                           # a fresh state: the e2e steps never meet a reset
         g.get_state(host)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
             g.set_state(host)
-            g.step(w.cfl * w.dx / g.max_wavespeed())
+            if ss:
+                ss.exchange()
+            solver.step(w.cfl * w.dx / solver.max_wavespeed())
             g.get_state(host)
         barrier()
         t_e2e = (time.perf_counter() - t0) / args.e2e_steps
-        t_e2e = reduce_max(t_e2e, world, dev)
-        nbytes = 5 * cells * 4
+        t_e2e = reduce_max(t_e2e, world, rdev)
+        nbytes = 5 * lw.n_cells * 4
         e2e = {"value": job_numbers(t_e2e * 1e3, cells, world)["grind_ns"], "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 8, "ms_per_step": t_e2e * 1e3, "pinned_host": pinned}
 
@@ -301,7 +350,10 @@ def run_ours(args):
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
                       "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
-                      "cfl": w.cfl, "parallelism": "replicas only" if world > 1 else "single GPU",
+                      "cfl": w.cfl,
+                      "parallelism": ("z slabs: %d ranks x %d owned planes + 8 overlap planes per neighbour, one halo "
+                                      "exchange per RK stage (%s)" % (world, w.nz, ss.exchange_kind)) if ss else "single GPU",
+                      "exchange_ms_per_step": (t_ex[0] * 1e3 / nprof) if ss else 0.0,
                       "l2": "inputs larger than L2 (no flush needed)" if cells * 4 > (126 << 20) else "inputs fit L2",
                       "wavespeed_query_every_step": True, "resets": resets[0]},
            "cell_updates_per_s": job["cell_updates_per_s"],
@@ -311,6 +363,8 @@ def run_ours(args):
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
+        barrier()
+        ss.close()
         dist.destroy_process_group()
 
 

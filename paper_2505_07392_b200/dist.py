@@ -64,11 +64,26 @@ class SlabSolver:
     def _connect_ipc(self):
         mine = self.solver.export_fields()
         blobs = _gather_bytes(bytes(mine), self.group)
-        for t in self._recv:
-            peer = igr.Export.from_buffer_copy(blobs[t.peer])
-            base = igr.ipc_open(peer)
-            self._opened.append(base)
-            self.solver.set_neighbor(t.side, peer, base, t.dst, t.src, t.count)
+        ok = 1
+        try:
+            for t in self._recv:
+                peer = igr.Export.from_buffer_copy(blobs[t.peer])
+                base = igr.ipc_open(peer)
+                self._opened.append(base)
+                self.solver.set_neighbor(t.side, peer, base, t.dst, t.src, t.count)
+        except igr.IgrError:
+            ok = 0
+        # all ranks use the same kind of exchange: if CUDA IPC was refused anywhere, nobody uses it
+        dev = self.solver.device if dist.get_backend(self.group) == "nccl" else "cpu"
+        flag = torch.tensor([ok], dtype=torch.int32, device=dev)
+        dist.all_reduce(flag, op=dist.ReduceOp.MIN, group=self.group)
+        if int(flag.item()) == 0:
+            for side in (0, 1):
+                self.solver.set_neighbor(side, None, None, 0, 0, 0)
+            for b in self._opened:
+                igr.ipc_close(b)
+            self._opened = []
+            self.exchange_kind = "sendrecv"
 
     def connect_local(self, solvers):
         """exchange="local": `solvers[r]` is the SlabSolver of rank r in this process."""
@@ -104,6 +119,8 @@ class SlabSolver:
     def _barrier(self):
         if self.exchange_kind in ("ipc", "sendrecv"):
             dist.barrier(group=self.group)
+            if dist.get_backend(self.group) == "nccl":
+                torch.cuda.synchronize(self.solver.device)    # the barrier itself is a device collective
 
     def exchange(self):
         """After a stage: every rank's overlap and ghost planes <- the neighbours' owned planes."""

@@ -1,4 +1,4 @@
-"""The N > 1 plumbing of bench.py (replicas only) on CPU: two gloo ranks
+"""The N > 1 timing plumbing of bench.py (the slab exchange itself is tests/test_slab_cpu.py) on CPU: two gloo ranks
 rendezvous on 127.0.0.1, the per-rank times are max-reduced and the whole-job numbers follow."""
 import os
 import socket
@@ -33,7 +33,7 @@ def _worker(rank, world, port, out):
         dist.destroy_process_group()
 
 
-def test_two_gloo_ranks_max_reduce_and_replica_metric():
+def test_two_gloo_ranks_max_reduce_and_job_metric():
     world, port = 2, _free_port()
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
@@ -47,7 +47,7 @@ def test_two_gloo_ranks_max_reduce_and_replica_metric():
     for rank, ms, grind, cups in res:
         assert ms == 20.0                                   # max over ranks
         assert grind == pytest.approx(20.0 * 1e6 / (2000 * 15))
-        assert cups == pytest.approx(2000 / 20e-3)          # aggregate over both replicas
+        assert cups == pytest.approx(2000 / 20e-3)          # aggregate over both ranks
 
 
 def test_single_rank_needs_no_process_group():
@@ -55,5 +55,5 @@ def test_single_rank_needs_no_process_group():
     import bench
     assert bench.reduce_max(3.5, 1) == 3.5
     one, two = bench.job_numbers(10.0, 1000, 1), bench.job_numbers(10.0, 1000, 2)
-    assert two["cell_updates_per_s"] == 2 * one["cell_updates_per_s"]     # weak scaling of replicas
+    assert two["cell_updates_per_s"] == 2 * one["cell_updates_per_s"]     # weak scaling
     assert two["grind_ns"] == pytest.approx(one["grind_ns"] / 2)
