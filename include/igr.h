@@ -188,8 +188,12 @@ int igr_ipc_close(void *peer_base);
 int igr_set_neighbor(igr_solver *s, int side, const igr_export *peer, const void *peer_base,
                      int dst_plane, int src_plane, int count);
 /* enqueue the copies of q (5 fields of the current buffer) and Sigma from every registered neighbour
- * on the solver's stream; invalidates the cached wave speed */
+ * on the solver's stream; drops the cached wave speed if a plane that entered it is overwritten */
 int igr_pull_halo(igr_solver *s);
+/* planes [k0, k1) (0 <= k0 < k1 <= nz) that enter igr_max_wavespeed and the fused stage-3 reduction;
+ * default all.  A slab restricts it to its owned planes: the overlap planes are only exact right after a
+ * pull, and the max over ranks of the owned maxima is the global maximum. */
+int igr_set_wave_range(igr_solver *s, int k0, int k1);
 
 /* ---- measurement hooks (bench.py).  Rows: 0 halo_bc, 1 sigma_source, 2 jacobi (sweeps + Sigma
  * ghosts), 3 rhs, 4 rk_update, 5 max_wavespeed (standalone reduction). */

@@ -34,6 +34,7 @@ Grid make_grid(int nx, int ny, int nz, int storage, const int32_t *faces)
     g.sz = (long long)g.px * g.py;
     g.np = g.sz * g.pz;
     for (int f = 0; f < 6; ++f) g.bc[f] = faces ? faces[f] : 0;
+    g.wk0 = 0; g.wk1 = nz;
     return g;
 }
 
@@ -670,7 +671,19 @@ int igr_pull_halo(igr_solver *s)
         IGR_CUDA_OK(cudaMemcpyAsync((char *)s->sig[s->sig_cur] + doff, nb.base + nb.desc.sig_offset[s->sig_cur] + soff, n,
                                     cudaMemcpyDeviceToDevice, s->stream));
     }
-    s->wave_valid = false;          // the overlap planes changed: the cached wave speed is stale
+    // the cached wave speed stays valid if no plane that entered it was overwritten (igr_set_wave_range)
+    for (int side = 0; side < 2; ++side) {
+        const igr_solver::Neighbor &nb = s->nb[side];
+        if (nb.active && nb.dst < s->g.wk1 && nb.dst + nb.count > s->g.wk0) s->wave_valid = false;
+    }
+    return IGR_OK;
+}
+
+int igr_set_wave_range(igr_solver *s, int k0, int k1)
+{
+    if (!s || k0 < 0 || k1 > s->g.nz || k0 >= k1) return IGR_ERR_ARG;
+    s->g.wk0 = k0; s->g.wk1 = k1;
+    s->wave_valid = false;
     return IGR_OK;
 }
 

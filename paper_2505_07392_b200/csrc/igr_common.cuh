@@ -21,6 +21,7 @@ struct Grid {
     long long sy, sz;      // strides in elements: sy = px, sz = px * py
     long long np;          // px * py * pz
     int bc[6];             // IGR_BC_* per face
+    int wk0, wk1;          // planes [wk0, wk1) that enter the wave-speed reduction (default: all; slabs: owned)
     __host__ __device__ long long idx(int i, int j, int k) const {   // interior-relative indices
         return (long long)(i + gx) + sy * (long long)(j + IGR_NG) + sz * (long long)(k + IGR_NG);
     }

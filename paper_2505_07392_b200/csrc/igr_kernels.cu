@@ -540,7 +540,8 @@ __global__ void k_rk_update(Grid g, StagePtrs qn, StagePtrs qs, StagePtrs qo, co
             stf((T *)qo.f[c] + id, o[c]);
             if (WAVE) o[c] = ldf((const T *)qo.f[c] + id);      // wave speed of the STORED state
         }
-        if (WAVE) vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], gamma, bad));
+        if (WAVE && k >= g.wk0 && k < g.wk1)
+            vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], gamma, bad));
     }
     if (WAVE) block_reduce_wave(vmax, bad, wave);
 }
@@ -569,6 +570,7 @@ __global__ void k_wavespeed(Grid g, StagePtrs q, float gamma, WaveResult *wave)
          t += (long long)gridDim.x * blockDim.x) {
         int i = (int)(t % g.nx); long long r = t / g.nx;
         int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        if (k < g.wk0 || k >= g.wk1) continue;
         const long long id = g.idx(i, j, k);
         vmax = fmaxf(vmax, wavespeed_of(ldf((const T *)q.f[0] + id), ldf((const T *)q.f[1] + id),
                                         ldf((const T *)q.f[2] + id), ldf((const T *)q.f[3] + id),

@@ -435,7 +435,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
                     o[c] = __fmaf_rn(a.beta, __fmaf_rn(a.dt, r[c], __fsub_rn(qs, qn)), qn);
                     stf(reinterpret_cast<T *>(a.qout[c]) + id, o[c]);
                 }
-                if (a.wave) {
+                if (a.wave && kz0 + t >= g.wk0 && kz0 + t < g.wk1) {
                     if (sizeof(T) < 4) {
 #pragma unroll
                         for (int c = 0; c < 5; ++c) o[c] = ldf(reinterpret_cast<const T *>(a.qout[c]) + id);

@@ -260,7 +260,7 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
                 o[c] = __fmaf_rn(a.beta, __fmaf_rn(a.dt, rr[c], __fsub_rn(qs, qn)), qn);
                 stf(reinterpret_cast<T *>(a.qout[c]) + id, o[c]);
             }
-            if (a.wave) {
+            if (a.wave && kz0 + t >= g.wk0 && kz0 + t < g.wk1) {
                 if (sizeof(T) < 4) {
 #pragma unroll
                     for (int c = 0; c < 5; ++c) o[c] = ldf(reinterpret_cast<const T *>(a.qout[c]) + id);

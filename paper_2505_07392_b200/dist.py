@@ -54,6 +54,8 @@ class SlabSolver:
         device = device or "cuda:%d" % torch.cuda.current_device()
         # the library owns its memory (cudaMalloc) so that the allocation has an IPC handle of its own
         self.solver = igr.Solver.for_workload(self.slab.local, device=device, own_workspace=False, **solver_kw)
+        if self.nranks > 1:                       # CFL reduction over the owned planes only
+            self.solver.set_wave_range(self.slab.own_lo, self.slab.own_hi)
         self._opened = []
         self._recv = S.receives(self.slab, lambda r: self.peer_slabs[r])
         self._send = S.sends(self.slab, lambda r: self.peer_slabs[r])
@@ -166,7 +168,6 @@ class SlabSolver:
                 for v in views:
                     v.copy_(buf[o:o + v.numel()], non_blocking=False)
                     o += v.numel()
-        self.solver.pull_halo()                    # no neighbour registered: only drops the cached wave speed
 
     def max_wavespeed(self):
         """Global maximum of |u_d| + c (CFL condition): local reduction kernel, then max over ranks."""

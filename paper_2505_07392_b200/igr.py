@@ -26,7 +26,7 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_sync", "igr_last_error", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs",
            "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
            "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity", "igr_stage",
-           "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo"]
+           "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo", "igr_set_wave_range"]
 
 
 class IgrError(RuntimeError):
@@ -96,6 +96,7 @@ def lib():
         L.igr_ipc_close.argtypes = [vp]
         L.igr_set_neighbor.argtypes = [vp, C.c_int, C.POINTER(Export), vp, C.c_int, C.c_int, C.c_int]
         L.igr_pull_halo.argtypes = [vp]
+        L.igr_set_wave_range.argtypes = [vp, C.c_int, C.c_int]
         L.igr_last_error.argtypes = [vp]
         L.igr_last_error.restype = C.c_char_p
         _lib = L
@@ -276,6 +277,9 @@ class Solver:
 
     def pull_halo(self):
         self._check(lib().igr_pull_halo(self._h))
+
+    def set_wave_range(self, k0, k1):
+        self._check(lib().igr_set_wave_range(self._h, int(k0), int(k1)))
 
     ROWS = ("halo_bc", "sigma_source", "jacobi", "rhs", "rk_update", "max_wavespeed")
 

@@ -96,13 +96,14 @@ def local_state(w, slab, device="cpu", dtype=None):
     import torch
     dtype = dtype or torch.float32
     chunk = max(1, (1 << 24) // (w.nx * w.ny))
-    parts, k = [], slab.e0
+    out = torch.empty((5, slab.e1 - slab.e0, w.ny, w.nx), dtype=dtype, device=torch.device(device))
+    k = slab.e0
     while k < slab.e1:
         g = k % w.nz                                  # wrapped start
         n = min(slab.e1 - k, w.nz - g, chunk)
-        parts.append(_state_slab(w, device, dtype, g, n))
+        out[:, k - slab.e0:k - slab.e0 + n] = _state_slab(w, device, dtype, g, n)
         k += n
-    return torch.cat(parts, dim=1)
+    return out
 
 
 @dataclass
