@@ -227,8 +227,9 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
 // footnote L252) with second-order central differences of the cell-centred velocity u = m/rho
 // (L132; Alg. 1).  G_ab = d u_a / d x_b.
 // Streaming form: a CTA owns a 32 x 8 column of cells and marches along z.  Each cell's velocity is
-// computed once (one reciprocal per cell) and shared: in-plane neighbours through a triple-buffered
-// shared-memory plane with a one-cell halo, z neighbours in registers.  4 loads + 1 store per cell.
+// computed once (one reciprocal per cell) and shared: in-plane neighbours through a ring of five
+// shared-memory planes with a one-cell halo (two planes enter per barrier), z neighbours in registers.
+// 4 loads + 1 store per cell.
 constexpr int SRC_TX = 32, SRC_TY = 8, SRC_ZC = 128;
 
 // GRAD: the same gradients also give the viscous stress tau (eq. 5; NEXT-1, igr_viscous.cuh), stored
@@ -239,7 +240,8 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
                                                             float lam2)
 {
     constexpr int PW = SRC_TX + 2, PH = SRC_TY + 2, PN = PW * PH;
-    __shared__ float U[3][3][PN];                            // three plane buffers: one barrier per step
+    constexpr int NB = 5;                                    // plane buffers: two planes per barrier
+    __shared__ float U[NB][3][PN];
     const T *rho = (const T *)q.f[0];
     const T *m[3] = { (const T *)q.f[1], (const T *)q.f[2], (const T *)q.f[3] };
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, tid = threadIdx.x;
@@ -256,44 +258,30 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
     if (tid < 2 * SRC_TX + 2 * SRC_TY) {
         int hx, hy;
         if (tid < 2 * SRC_TX) { hx = tid & 31; hy = (tid >> 5) ? SRC_TY : -1; }
-        else { const int t = tid - 2 * SRC_TX; hy = t & 7; hx = (t >> 3) ? SRC_TX : -1; }
+        else { const int t = tid - 2 * SRC_TX; hy = t % SRC_TY; hx = (t / SRC_TY) ? SRC_TX : -1; }
         const int hi = min(max(x0 + hx, -1), g.nx), hj = min(max(y0 + hy, -1), g.ny);
         hpos = (hy + 1) * PW + hx + 1;
         hcol = (unsigned)(hi + g.gx) + (unsigned)g.sy * (unsigned)(hj + IGR_NG);
     }
-    // raw loads of plane k (own column + halo cell) are issued one step before they are consumed
-    float rw[4], hw[4];
-    auto fetch = [&](int k) {
+    // raw loads of a plane (own column + halo cell) are issued one iteration before they are consumed
+    struct Raw { float r[4], h[4]; };
+    auto fetch = [&](int k, Raw &w) {
         const unsigned zo = usz * (unsigned)(min(k, g.nz) + IGR_NG);
-        rw[0] = ldf(rho + col + zo); rw[1] = ldf(m[0] + col + zo); rw[2] = ldf(m[1] + col + zo); rw[3] = ldf(m[2] + col + zo);
+        w.r[0] = ldf(rho + col + zo); w.r[1] = ldf(m[0] + col + zo); w.r[2] = ldf(m[1] + col + zo); w.r[3] = ldf(m[2] + col + zo);
         if (hpos >= 0) {
-            hw[0] = ldf(rho + hcol + zo); hw[1] = ldf(m[0] + hcol + zo); hw[2] = ldf(m[1] + hcol + zo); hw[3] = ldf(m[2] + hcol + zo);
+            w.h[0] = ldf(rho + hcol + zo); w.h[1] = ldf(m[0] + hcol + zo); w.h[2] = ldf(m[1] + hcol + zo); w.h[3] = ldf(m[2] + hcol + zo);
         }
     };
-    auto put_plane = [&](int buf, float &u, float &v, float &w) {          // fetched plane -> velocities
-        const float ir = __fdividef(1.0f, rw[0]);
-        u = rw[1] * ir; v = rw[2] * ir; w = rw[3] * ir;
-        U[buf][0][own] = u; U[buf][1][own] = v; U[buf][2][own] = w;
+    auto put_plane = [&](int buf, const Raw &w, float v[3]) {               // fetched plane -> velocities
+        const float ir = __fdividef(1.0f, w.r[0]);
+        v[0] = w.r[1] * ir; v[1] = w.r[2] * ir; v[2] = w.r[3] * ir;
+        U[buf][0][own] = v[0]; U[buf][1][own] = v[1]; U[buf][2][own] = v[2];
         if (hpos >= 0) {
-            const float hr = __fdividef(1.0f, hw[0]);
-            U[buf][0][hpos] = hw[1] * hr; U[buf][1][hpos] = hw[2] * hr; U[buf][2][hpos] = hw[3] * hr;
+            const float hr = __fdividef(1.0f, w.h[0]);
+            U[buf][0][hpos] = w.h[1] * hr; U[buf][1][hpos] = w.h[2] * hr; U[buf][2][hpos] = w.h[3] * hr;
         }
     };
-    float dn[3], ce[3], up[3];                               // own column at planes k-1, k, k+1
-    fetch(kz0 - 1);
-    {
-        const float ir = __fdividef(1.0f, rw[0]);
-        dn[0] = rw[1] * ir; dn[1] = rw[2] * ir; dn[2] = rw[3] * ir;
-    }
-    fetch(kz0);
-    put_plane(kz0 % 3, ce[0], ce[1], ce[2]);
-    fetch(kz0 + 1);
-    for (int t = 0; t < nkz; ++t) {
-        const int k = kz0 + t;
-        put_plane((k + 1) % 3, up[0], up[1], up[2]);         // next plane (the ghost plane at the top)
-        fetch(k + 2);                                        // lands during this step
-        __syncthreads();
-        const float (*P)[PN] = U[k % 3];
+    auto emit = [&](int k, const float (*P)[PN], const float dn[3], const float up[3]) {
         float G[3][3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
@@ -317,8 +305,33 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
                 tp.t[IGR_TAU_ZZ][id] = mu2 * G[2][2] + lt;
             }
         }
+    };
+    // own column at planes k-1, k (dn, ce) and the two planes that enter per iteration (u1, u2)
+    float dn[3], ce[3], u1[3], u2[3];
+    Raw A, B;
+    fetch(kz0 - 1, A);
+    {
+        const float ir = __fdividef(1.0f, A.r[0]);
+        dn[0] = A.r[1] * ir; dn[1] = A.r[2] * ir; dn[2] = A.r[3] * ir;
+    }
+    fetch(kz0, A);
+    int bc = 0;                                              // buffer of plane k (k = kz0 + t), mod NB
+    put_plane(bc, A, ce);
+    fetch(kz0 + 1, A);
+    fetch(kz0 + 2, B);
+    for (int t = 0; t < nkz; t += 2) {
+        const int k = kz0 + t;
+        const int b1 = (bc + 1 >= NB) ? bc + 1 - NB : bc + 1, b2 = (bc + 2 >= NB) ? bc + 2 - NB : bc + 2;
+        put_plane(b1, A, u1);                                // plane k + 1
+        put_plane(b2, B, u2);                                // plane k + 2 (ghost plane at the top)
+        fetch(k + 3, A);                                     // land during this iteration
+        fetch(k + 4, B);
+        __syncthreads();                                     // one barrier per two planes
+        emit(k, U[bc], dn, u1);
+        if (t + 1 < nkz) emit(k + 1, U[b1], ce, u2);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { dn[a] = ce[a]; ce[a] = up[a]; }
+        for (int a = 0; a < 3; ++a) { dn[a] = u1[a]; ce[a] = u2[a]; }
+        bc = b2;
     }
 }
 
