@@ -93,7 +93,9 @@ typedef struct {
 
 typedef struct igr_solver igr_solver;
 
-/* Device bytes a solver of this size needs (for igr_options.workspace). */
+/* Device bytes a solver of this size needs (for igr_options.workspace).  A fused tiled solver keeps no RHS
+ * array r[5] at rest (18 fields); it allocates one with cudaMalloc the first time igr_rhs, igr_rk_update,
+ * igr_get_rhs or a viscous step needs it (IGR_ERR_ALLOC if that fails). */
 size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt);
 
 /* Create a solver.  dx: uniform spacing in all directions; gamma > 1: ideal-gas exponent (eq. 4);

@@ -41,17 +41,21 @@ Grid make_grid(int nx, int ny, int nz, int storage, const int32_t *faces)
 struct Layout {
     size_t q_bytes, f_bytes;        // one padded field in storage type / in fp32
     int n_state;                    // state buffers (2 unfused, 3 fused)
+    int n_r;                        // r fields inside the workspace (5, or 0: allocated on first use)
     size_t total;
 };
 
-Layout make_layout(const Grid &g, int storage, int fused)
+Layout make_layout(const Grid &g, int storage, int fused, int variant)
 {
     Layout L;
     L.q_bytes = align_up((size_t)g.np * elem_size(storage), kAlign);
     L.f_bytes = align_up((size_t)g.np * 4, kAlign);
     L.n_state = fused ? 3 : 2;
-    // states + Sigma x2 (storage type) + b + r[5] (fp32) + staging + wave result
-    L.total = (size_t)L.n_state * 5 * L.q_bytes + 2 * L.q_bytes + 6 * L.f_bytes + kStageBytes + kAlign;
+    // the fused tiled step never materialises r: it is allocated only if an unfused row, igr_get_rhs or
+    // the viscous path asks for it (5 fp32 fields less: 18 instead of 23 fields at rest)
+    L.n_r = (fused && variant == IGR_VARIANT_TILED) ? 0 : 5;
+    // states + Sigma x2 (storage type) + b + r[n_r] (fp32) + staging + wave result
+    L.total = (size_t)L.n_state * 5 * L.q_bytes + 2 * L.q_bytes + (1 + L.n_r) * L.f_bytes + kStageBytes + kAlign;
     return L;
 }
 
@@ -78,6 +82,7 @@ struct igr_solver {
     std::vector<void *> bc_allocs;   // device arrays of the inflow faces
     std::string err;
     double mu = 0, zeta = 0;         // viscosity (NEXT-1); 0, 0: inviscid
+    float *r_owned = nullptr;        // r[5] when it is not part of the workspace (ensure_r)
     float *tau = nullptr;            // six stress fields (allocated by igr_set_viscosity; igr_viscous.cuh)
     ViscTileMaps vmaps;              // TMA maps of the tiled viscous kernel
     struct Neighbor {                // NEXT-2: neighbouring slab on z- / z+ (igr_set_neighbor)
@@ -219,6 +224,21 @@ struct RowTimer {
     ~RowTimer() { if (s->profile) cudaEventRecord(s->ev.back(), s->stream); }
 };
 
+// r[5] of a fused tiled solver is not part of the workspace: allocate it on first use
+int ensure_r(igr_solver *s)
+{
+    if (s->r[0]) return IGR_OK;
+    const size_t fb = align_up((size_t)s->g.np * 4, kAlign);
+    if (cudaMalloc((void **)&s->r_owned, 5 * fb) != cudaSuccess) {
+        cudaGetLastError();
+        s->r_owned = nullptr;
+        return s->fail(IGR_ERR_ALLOC, "cudaMalloc of the RHS fields failed");
+    }
+    IGR_CUDA_OK(cudaMemsetAsync(s->r_owned, 0, 5 * fb, s->stream));
+    for (int c = 0; c < 5; ++c) s->r[c] = (float *)((char *)s->r_owned + c * fb);
+    return IGR_OK;
+}
+
 int finish(igr_solver *s, const char *what)
 {
     cudaError_t e = cudaGetLastError();
@@ -238,7 +258,7 @@ size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt)
     const int fused = opt ? opt->fused : 0;
     if (storage < 0 || storage > 2) return 0;
     Grid g = make_grid(nx, ny, nz, storage, nullptr);
-    return make_layout(g, storage, fused).total;
+    return make_layout(g, storage, fused, opt ? opt->variant : 0).total;
 }
 
 int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
@@ -275,7 +295,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
     s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
     s->g = make_grid(nx, ny, nz, storage, bc->face);
-    const Layout L = make_layout(s->g, storage, s->fused);
+    const Layout L = make_layout(s->g, storage, s->fused, s->variant);
     if (opt && opt->workspace) {
         if (opt->workspace_bytes < L.total || ((uintptr_t)opt->workspace % kAlign) != 0) {
             delete s;
@@ -299,7 +319,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->sig[0] = p; p += L.q_bytes;
     s->sig[1] = p; p += L.q_bytes;
     s->b = (float *)p; p += L.f_bytes;
-    for (int c = 0; c < 5; ++c) { s->r[c] = (float *)p; p += L.f_bytes; }
+    for (int c = 0; c < L.n_r; ++c) { s->r[c] = (float *)p; p += L.f_bytes; }
     s->stage = (float *)p; p += kStageBytes;
     s->wave = (WaveResult *)p;
     int rc = build_inflow(s, bc);
@@ -321,6 +341,7 @@ void igr_destroy(igr_solver *s)
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     if (s->tau) cudaFree(s->tau);
+    if (s->r_owned) cudaFree(s->r_owned);
     for (void *p : s->bc_allocs) cudaFree(p);
     if (s->owns_base && s->base) cudaFree(s->base);
     delete s;
@@ -399,6 +420,7 @@ int igr_set_source(igr_solver *s, const float *f)
 int igr_get_rhs(igr_solver *s, float *r)
 {
     if (!s || !r) return IGR_ERR_ARG;
+    { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
     for (int c = 0; c < 5; ++c) {
         int rc = field_out(s, s->r[c], r + c * n, IGR_STORE_F32);
@@ -480,6 +502,7 @@ int igr_jacobi(igr_solver *s)
 int igr_rhs(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
+    { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     RowTimer t(s, 3, 1);
     RhsParams p;
     p.gamma = (float)s->gamma; p.inv_dx = (float)(1.0 / s->dx); p.order = s->order;
@@ -513,6 +536,7 @@ int igr_rhs(igr_solver *s)
 int igr_rk_update(igr_solver *s, int stage, double dt)
 {
     if (!s || stage < 1 || stage > 3) return IGR_ERR_ARG;
+    { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     const float beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
     StagePtrs &A = s->st[0], &B = s->st[1];
     RowTimer t(s, 4, 1);
@@ -561,6 +585,7 @@ int igr_stage(igr_solver *s, int stage, double dt)
                 if (stage == 3) a.wave = s->wave;
                 launch_rhs_tile(s->g, s->storage, s->order, true, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
             } else {
+                if ((rc = ensure_r(s)) != IGR_OK) return rc;
                 for (int c = 0; c < 5; ++c) a.r[c] = s->r[c];
                 launch_rhs_tile(s->g, s->storage, s->order, false, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
                 launch_halo_fields(s->g, s->tau, 6, s->stream);

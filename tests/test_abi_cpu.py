@@ -37,8 +37,12 @@ def test_workspace_bytes_counts_the_fields(lib):
     opt.storage = igr.STORE_F16
     b16 = lib.igr_workspace_bytes(n, n, n, C.byref(opt))
     assert b16 < b32
-    opt.fused = 1
-    assert lib.igr_workspace_bytes(n, n, n, C.byref(opt)) > b16
+    opt.fused = 1                                             # third state buffer, but r[5] is not resident
+    opt.storage = igr.STORE_F32
+    bf = lib.igr_workspace_bytes(n, n, n, C.byref(opt))
+    assert 18 * field <= bf <= 18 * field + (80 << 20)       # 15 q + 2 Sigma + b, + staging
+    opt.variant = igr.VARIANT_SIMPLE                          # the simple kernels always run the unfused rows
+    assert lib.igr_workspace_bytes(n, n, n, C.byref(opt)) >= 23 * field
     assert lib.igr_workspace_bytes(0, n, n, C.byref(opt)) == 0
 
 
