@@ -215,12 +215,23 @@ def run_ours(args):
         q0 = S.local_state(wg, ss.slab, device=dev)
     else:
         g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
-        q0 = W.state(w, device=dev)
+        # the fp32 copy of the initial state stays on the device for restarts only if it fits beside the solver
+        free_b = torch.cuda.mem_get_info(torch.device(dev))[0]
+        q0 = W.state(w, device=dev) if free_b > 5 * cells * 4 + (12 << 30) else None
     if args.mu > 0 or args.zeta > 0:
         g.set_viscosity(args.mu, args.zeta)
+    filled = [False]
 
     def load_initial():
-        g.set_state(q0)
+        if q0 is not None:
+            g.set_state(q0)
+        else:                             # slab by slab through igr_set_state_planes (large grids)
+            nk = max(1, (1 << 24) // (w.nx * w.ny))
+            for k0 in range(0, w.nz, nk):
+                g.set_state_planes(k0, W.state_planes(w, k0, min(nk, w.nz - k0), device=dev))
+            if filled[0]:                 # restart: Sigma back to zero (a fresh solver has it zero already)
+                g.set_sigma(torch.zeros((w.nz, w.ny, w.nx), dtype=torch.float32, device=dev))
+            filled[0] = True
         if ss:
             ss.exchange()                 # ghost planes from the neighbours
 

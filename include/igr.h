@@ -112,6 +112,12 @@ void igr_destroy(igr_solver *s);
 int igr_set_state(igr_solver *s, const float *q);
 /* Copy the current state out; synchronises.  IGR_ERR_NONFINITE is NOT raised here. */
 int igr_get_state(igr_solver *s, float *q);
+/* The same for the planes [k0, k0 + nk) only, q: [5][nk][ny][nx] (host or device).  For grids whose whole
+ * fp32 state does not fit beside the solver (180 GB: 1280^3 in fp32, 1536^3 with 2-byte storage), and
+ * for slab-wise I/O.  igr_set_state_planes does NOT reset Sigma (igr_set_state does) and is refused in
+ * the middle of a step; IGR_ERR_ARG for a range outside [0, nz). */
+int igr_set_state_planes(igr_solver *s, int k0, int nk, const float *q);
+int igr_get_state_planes(igr_solver *s, int k0, int nk, float *q);
 /* Sigma is part of a restart because of the warm start (L130, L138).  f: [nz][ny][nx]. */
 int igr_set_sigma(igr_solver *s, const float *f);
 int igr_get_sigma(igr_solver *s, float *f);

@@ -170,38 +170,41 @@ bool is_device_pointer(const void *p)
 }
 
 // copy one user field (interior, fp32, host or device) into / out of a padded field
-int field_in(igr_solver *s, const float *user, void *field, int storage)
+// (planes [kfirst, kfirst + nplanes) of the field; `user` holds exactly those planes; nplanes < 0: all)
+int field_in(igr_solver *s, const float *user, void *field, int storage, int kfirst = 0, int nplanes = -1)
 {
     const Grid &g = s->g;
+    if (nplanes < 0) nplanes = g.nz;
     if (is_device_pointer(user)) {
-        launch_unpack_field(g, storage, user, field, 0, g.nz, s->stream);
+        launch_unpack_field(g, storage, user, field, kfirst, nplanes, s->stream);
         return IGR_OK;
     }
     const size_t plane = (size_t)g.nx * g.ny * 4;
     int chunk = (int)(kStageBytes / plane);
     if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
-    for (int k0 = 0; k0 < g.nz; k0 += chunk) {
-        const int nk = (g.nz - k0 < chunk) ? g.nz - k0 : chunk;
+    for (int k0 = 0; k0 < nplanes; k0 += chunk) {
+        const int nk = (nplanes - k0 < chunk) ? nplanes - k0 : chunk;
         IGR_CUDA_OK(cudaMemcpyAsync(s->stage, user + (size_t)k0 * g.nx * g.ny, nk * plane,
                                     cudaMemcpyHostToDevice, s->stream));
-        launch_unpack_field(g, storage, s->stage, field, k0, nk, s->stream);
+        launch_unpack_field(g, storage, s->stage, field, kfirst + k0, nk, s->stream);
     }
     return IGR_OK;
 }
 
-int field_out(igr_solver *s, const void *field, float *user, int storage)
+int field_out(igr_solver *s, const void *field, float *user, int storage, int kfirst = 0, int nplanes = -1)
 {
     const Grid &g = s->g;
+    if (nplanes < 0) nplanes = g.nz;
     if (is_device_pointer(user)) {
-        launch_pack_field(g, storage, field, user, 0, g.nz, s->stream);
+        launch_pack_field(g, storage, field, user, kfirst, nplanes, s->stream);
         return IGR_OK;
     }
     const size_t plane = (size_t)g.nx * g.ny * 4;
     int chunk = (int)(kStageBytes / plane);
     if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
-    for (int k0 = 0; k0 < g.nz; k0 += chunk) {
-        const int nk = (g.nz - k0 < chunk) ? g.nz - k0 : chunk;
-        launch_pack_field(g, storage, field, s->stage, k0, nk, s->stream);
+    for (int k0 = 0; k0 < nplanes; k0 += chunk) {
+        const int nk = (nplanes - k0 < chunk) ? nplanes - k0 : chunk;
+        launch_pack_field(g, storage, field, s->stage, kfirst + k0, nk, s->stream);
         IGR_CUDA_OK(cudaMemcpyAsync(user + (size_t)k0 * g.nx * g.ny, s->stage, nk * plane,
                                     cudaMemcpyDeviceToHost, s->stream));
         IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
@@ -371,6 +374,30 @@ int igr_set_state(igr_solver *s, const float *q)
     s->sig_cur = 0;
     s->wave_valid = false;
     return finish(s, "igr_set_state");
+}
+
+int igr_set_state_planes(igr_solver *s, int k0, int nk, const float *q)
+{
+    if (!s || !q || k0 < 0 || nk < 1 || k0 + nk > s->g.nz) return IGR_ERR_ARG;
+    if (s->cur != 0) return s->fail(IGR_ERR_ARG, "igr_set_state_planes: called in the middle of a step");
+    const size_t n = (size_t)s->g.nx * s->g.ny * nk;
+    for (int c = 0; c < 5; ++c) {
+        int rc = field_in(s, q + c * n, s->st[0].f[c], s->storage, k0, nk);
+        if (rc != IGR_OK) return rc;
+    }
+    s->wave_valid = false;
+    return finish(s, "igr_set_state_planes");
+}
+
+int igr_get_state_planes(igr_solver *s, int k0, int nk, float *q)
+{
+    if (!s || !q || k0 < 0 || nk < 1 || k0 + nk > s->g.nz) return IGR_ERR_ARG;
+    const size_t n = (size_t)s->g.nx * s->g.ny * nk;
+    for (int c = 0; c < 5; ++c) {
+        int rc = field_out(s, s->st[s->cur].f[c], q + c * n, s->storage, k0, nk);
+        if (rc != IGR_OK) return rc;
+    }
+    return igr_sync(s);
 }
 
 int igr_get_state(igr_solver *s, float *q)

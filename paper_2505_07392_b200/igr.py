@@ -26,7 +26,8 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_sync", "igr_last_error", "igr_halo_bc", "igr_sigma_source", "igr_jacobi", "igr_rhs",
            "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
            "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity", "igr_stage",
-           "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo", "igr_set_wave_range"]
+           "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo", "igr_set_wave_range", "igr_set_state_planes",
+           "igr_get_state_planes"]
 
 
 class IgrError(RuntimeError):
@@ -81,6 +82,8 @@ def lib():
                   "igr_set_source", "igr_get_rhs"):
             getattr(L, n).argtypes = [vp, fp]
         L.igr_get_padded.argtypes = [vp, C.c_int, fp]
+        L.igr_set_state_planes.argtypes = [vp, C.c_int, C.c_int, fp]
+        L.igr_get_state_planes.argtypes = [vp, C.c_int, C.c_int, fp]
         L.igr_max_wavespeed.argtypes = [vp, C.POINTER(C.c_double)]
         L.igr_step.argtypes = [vp, C.c_double]
         L.igr_rk_update.argtypes = [vp, C.c_int, C.c_double]
@@ -202,6 +205,16 @@ class Solver:
     def get_state(self, out=None):
         out = np.empty((5,) + self.shape, np.float32) if out is None else out
         self._check(lib().igr_get_state(self._h, _addr(out, (5,) + self.shape, True)))
+        return out
+
+    def set_state_planes(self, k0, q):
+        """q: [5][nk][ny][nx], planes k0 .. k0 + nk - 1 (Sigma is left as it is)."""
+        nk = int(q.shape[1])
+        self._check(lib().igr_set_state_planes(self._h, int(k0), nk, _addr(q, (5, nk, self.ny, self.nx))))
+
+    def get_state_planes(self, k0, nk, out=None):
+        out = np.empty((5, nk, self.ny, self.nx), np.float32) if out is None else out
+        self._check(lib().igr_get_state_planes(self._h, int(k0), int(nk), _addr(out, (5, nk, self.ny, self.nx), True)))
         return out
 
     def set_sigma(self, f):

@@ -100,6 +100,11 @@ def state(w, device="cpu", dtype=torch.float32, slab=None):
     return q
 
 
+def state_planes(w, k0, nk, device="cpu", dtype=torch.float32):
+    """Planes [k0, k0 + nk) of the initial state, [5][nk][ny][nx] (for grids filled slab by slab)."""
+    return _state_slab(w, device, dtype, k0, nk)
+
+
 def _state_slab(w, device, dtype, kz0, nk):
     dev = torch.device(device)
     gi, gj, gk = _index_grids(w, dev, kz0, nk)

@@ -156,3 +156,64 @@ def test_jets_run_stays_finite_and_positive():
     g.get_state(out)
     p = 0.4 * (out[4] - 0.5 * (out[1] ** 2 + out[2] ** 2 + out[3] ** 2) / out[0])
     assert torch.isfinite(out).all() and float(out[0].min()) > 0 and float(p.min()) > 0
+
+
+def _fill_by_planes(g, w):
+    nk = max(1, (1 << 24) // (w.nx * w.ny))
+    for k0 in range(0, w.nz, nk):
+        g.set_state_planes(k0, W.state_planes(w, k0, min(nk, w.nz - k0), device="cuda"))
+
+
+@pytest.mark.skipif(not FULL, reason="full-size configs disabled")
+@pytest.mark.parametrize("n,fmt", [(1280, "f32"), (1536, "f16")])
+def test_largest_grids_that_fit_one_b200(n, fmt):
+    """Maximum sizes: 1280^3 in fp32 (2.1e9 cells, 154 GB) and 1536^3 with fp16 storage (3.6e9 cells, 140 GB;
+    element offsets up to 3.7e9 of the 2^32 the kernels' unsigned offsets hold).  The state does not fit
+    beside the solver a second time, so it goes in and out by plane ranges.  One step, compared on the
+    48^3 block in the far (x+, y+, z+) corner, where the offsets are largest, through the
+    dependency-cone sub-box (27 cells per step)."""
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                                  # what earlier tests left in torch's cache
+    free_b = torch.cuda.mem_get_info()[0]
+    if free_b < (170 << 30):
+        pytest.skip("needs 170 GB of free device memory")
+    from test_gpu_storage import FMT, compare_stored
+    w = W.jets33(n=n)
+    size, pad = 48, 32
+    target = (n - size,) * 3
+    lo = tuple(t - pad for t in target)
+    hi = (n, n, n)
+    wb = W.subbox(w, lo, hi)
+    storage = igr.STORE_F32 if fmt == "f32" else FMT[fmt]["gpu"]
+    g = igr.Solver.for_workload(w, storage=storage, fused=1)
+    _fill_by_planes(g, w)
+    qb = W.state(wb).numpy()
+    # the sub-box generator reproduces the device-generated cut up to libm differences: hand the GPU's own
+    # planes of that region to the oracle
+    cut = g.get_state_planes(lo[2], hi[2] - lo[2])[:, :, lo[1]:hi[1], lo[0]:hi[0]]
+    if fmt == "f32":
+        np.testing.assert_allclose(cut, qb, rtol=1e-6, atol=1e-7)
+        ref = parity.oracle_for(wb)
+        ref.set_state(cut.astype(np.float64))
+    else:
+        # the stored planes are already rounded to fp16; the emulating oracle starts from the same values
+        qb32 = W.state_planes(w, lo[2], hi[2] - lo[2], device="cuda")[:, :, lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        ref = parity.oracle_for(wb, storage=FMT[fmt]["ref"])
+        ref.set_state(qb32.astype(np.float64))
+        assert np.array_equal(ref.get_state().astype(np.float32), cut)
+    dt = w.cfl * w.dx / g.max_wavespeed()
+    g.step(dt); ref.step(dt)
+    assert g.max_wavespeed() > 0                              # raises on a non-finite state
+    got = g.get_state_planes(target[2], size)[:, :, target[1]:, target[0]:]
+    want = ref.get_state()[:, pad:, pad:, pad:]
+    if fmt == "f32":
+        mx, l1 = parity.worst(got, want)
+        assert l1 <= 1e-3 and mx <= 1e-4, (mx, l1)
+    else:
+        same, within1, worst = compare_stored(got, want, FMT[fmt]["pbits"])
+        assert same >= 0.97 and within1 >= 0.999 and worst <= 8.0, (same, within1, worst)
+    g.close()
+    del g
+    gc.collect()
+    torch.cuda.empty_cache()
