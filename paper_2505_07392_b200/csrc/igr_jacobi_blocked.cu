@@ -5,8 +5,8 @@
 // sweeps (16 B per cell instead of 16 B per sweep).
 //
 // Design: 2.5-D streaming with a skewed pipeline of sweep levels.
-// A CTA of 1024 threads owns a 32 x 32 column region = (32-2NS)^2 output columns + an NS-wide halo
-// that is recomputed (the dependency cone of NS sweeps), and marches along z.  At step tau the plane
+// A CTA of 512 threads (two columns per thread) owns a 32 x 32 column region = (32-2NS)^2 output columns
+// + an NS-wide halo that is recomputed (the dependency cone of NS sweeps), and marches along z.  At step tau the plane
 // p0 enters; level l+1 (l = 0..NS-1) advances its iterate on plane p0-1-l from level l's planes
 // p0-2-l .. p0-l.  In-plane neighbours come from double-buffered shared-memory planes (one per
 // level), the z neighbours and all seven stencil coefficients of the NS planes in flight live in

@@ -101,6 +101,7 @@ class SlabSolver:
         for b in self._opened:
             igr.ipc_close(b)
         self._opened = []
+        self._barrier()                            # an exporter frees its memory only after every importer unmapped it
         self.solver.close()
 
     # ---- state
