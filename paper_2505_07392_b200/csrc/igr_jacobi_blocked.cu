@@ -139,9 +139,10 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
 #pragma unroll
         for (int cc = 0; cc < CPT; ++cc) {
             // (for 2-byte T the source address is rounded down to its 4-byte word)
-            cp4(st + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(rho + (off_r[cc] + zr)) & ~(uintptr_t)3));
+            constexpr uintptr_t WORD = (sizeof(T) == 4) ? ~(uintptr_t)0 : ~(uintptr_t)3;
+            cp4(st + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(rho + (off_r[cc] + zr)) & WORD));
             cp4(st + R * R + cc * NTHREADS, bsrc + (off_m[cc] + zm));
-            cp4(st + 2 * R * R + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(sin + (off_m[cc] + zm)) & ~(uintptr_t)3));
+            cp4(st + 2 * R * R + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(sin + (off_m[cc] + zm)) & WORD));
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
