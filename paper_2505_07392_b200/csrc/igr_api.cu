@@ -65,6 +65,7 @@ struct igr_solver {
     Grid g;
     int storage = 0, fused = 0, variant = 0, order = 5, n_jacobi = 5;
     RhsTileMaps maps;
+    JacobiMaps jmaps;                // TMA maps of the blocked Jacobi kernel
     double dx = 0, gamma = 0, alpha = 0;
     cudaStream_t stream = nullptr;
     char *base = nullptr;            // device memory (owned or caller's workspace)
@@ -294,6 +295,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->fused = opt ? (opt->fused != 0) : 0;
     s->variant = opt ? opt->variant : 0;
     s->maps.valid = false;
+    s->jmaps.valid = false;
     s->order = order; s->n_jacobi = n_jacobi;
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
     s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
@@ -330,6 +332,10 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     if (s->variant == IGR_VARIANT_TILED) {
         const char *msg = "";
         if (rhs_tile_make_maps(s->g, storage, s->st, L.n_state, s->sig, &s->maps, &msg) != 0) {
+            igr_destroy(s);
+            return IGR_ERR_CUDA;
+        }
+        if (jacobi_make_maps(s->g, storage, s->st, L.n_state, s->sig, s->b, &s->jmaps) != 0) {
             igr_destroy(s);
             return IGR_ERR_CUDA;
         }
@@ -506,11 +512,16 @@ int igr_jacobi(igr_solver *s)
         // temporally blocked: passes of up to 5 sweeps, each ONE read of rho, b, Sigma and one write
         static int maxns = -1;                   // IGR_JACOBI_MAXNS=1..5: sweeps per blocked pass (tuning)
         if (maxns < 0) { const char *e = getenv("IGR_JACOBI_MAXNS"); maxns = e ? atoi(e) : 5; if (maxns < 1 || maxns > 5) maxns = 5; }
+        static int no_tma = -1;                  // IGR_JACOBI_TMA=0: cp.async staging everywhere (tuning)
+        if (no_tma < 0) { const char *e = getenv("IGR_JACOBI_TMA"); no_tma = (e && atoi(e) == 0) ? 1 : 0; }
         const int npass = (s->n_jacobi + maxns - 1) / maxns;
         RowTimer t(s, 2, npass + 1);
         for (int left = s->n_jacobi; left > 0; left -= maxns) {
+            const bool tma = s->jmaps.valid && !no_tma;
             launch_jacobi_blocked(s->g, s->storage, left < maxns ? left : maxns, s->st[s->cur].f[0], s->b,
-                                  s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2, s->stream);
+                                  s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2,
+                                  tma ? &s->jmaps.rho[s->cur] : nullptr, tma ? &s->jmaps.b : nullptr,
+                                  tma ? &s->jmaps.sig[s->sig_cur] : nullptr, s->stream);
             s->sig_cur = 1 - s->sig_cur;
         }
         launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);

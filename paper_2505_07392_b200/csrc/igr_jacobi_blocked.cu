@@ -16,9 +16,38 @@
 // place of its outside neighbour.
 #include "igr_kernels.h"
 
+#include <cuda.h>
+#include <cstdlib>
 #include <type_traits>
 
 namespace {
+
+__device__ __forceinline__ uint32_t jb_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void jb_mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(jb_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void jb_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(jb_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void jb_mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "JB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra JB_DONE;\n"
+        "bra JB_WAIT;\n"
+        "JB_DONE:\n"
+        "}\n" ::"r"(jb_smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void jb_tma_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(jb_smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(jb_smem_u32(bar)) : "memory");
+}
 
 constexpr int R = 32;                       // region edge
 constexpr int cpt_small = 2;                // columns per thread for NS <= 3 (1 = 1024 threads: measured slower)
@@ -40,25 +69,33 @@ __device__ __forceinline__ int rho_index(int i, int n, bool periodic)
     return min(max(i, -1), n);
 }
 
-constexpr int PF = 3;                       // cp.async prefetch distance in planes
+constexpr int PF = 3;                       // prefetch distance in planes (cp.async or TMA)
+constexpr int SUB = (R + 4) * R;            // floats of one staged field: an fp32 TMA box of (R + 4) x R
 // CPT = columns per thread (rows ry and ry + R/CPT of the region).  NS = 4, 5: CPT = 2, 512 threads x
 // 128 registers hold the pipeline state (7 coefficients x NS planes + 2 NS iterate values per column);
 // CPT = 1 (1024 threads x 64 registers, no spills for NS <= 3) was measured slower and is not used.
 template <typename T, int NS, int CPT>
 __global__ void __launch_bounds__(R * R / CPT, 1)
-k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bsrc, const T *__restrict__ sin,
-                 T *__restrict__ sout, float k2, int zc)
+k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ CUtensorMap bmap,
+                 const __grid_constant__ CUtensorMap smap, int use_tma, Grid g, const T *__restrict__ rho,
+                 const float *__restrict__ bsrc, const T *__restrict__ sin, T *__restrict__ sout, float k2, int zc)
 {
     constexpr int OT = R - 2 * NS;
     constexpr int NTHREADS = R * R / CPT;
     constexpr int P = R + 2;                 // padded plane pitch: a border of one cell, so that the
     constexpr int PP = P * (R + 2);          // four in-plane neighbours are at constant offsets
-    extern __shared__ __align__(16) float jb_smem[];
-    float (*RHO)[PP] = reinterpret_cast<float (*)[PP]>(jb_smem);                       // [2][PP]
-    float (*SP)[2][PP] = reinterpret_cast<float (*)[2][PP]>(jb_smem + 2 * PP);          // [NS][2][PP]
-    // fp32 storage: incoming planes are staged by cp.async PF steps ahead (ring of PF + 1 stages of
-    // rho, b, Sigma for the R*R columns); each thread reads back only what it copied itself
-    float *STG = jb_smem + (2 + 2 * NS) * PP;                                           // [PF+1][3][R*R]
+    extern __shared__ __align__(128) float jb_smem[];
+    // incoming planes are staged PF steps ahead into a ring of PF + 1 slots of (rho, b, Sigma) for the
+    // R*R columns.  A region that lies inside the domain in x and y is a plain box of the padded arrays:
+    // ONE thread issues three TMA loads per plane (mbarrier completion).  Regions that reach over the
+    // domain boundary gather through the BC index map with one 4-byte cp.async per column and field
+    // (each thread reads back only what it copied itself).
+    // A TMA box must start on a 16-byte boundary of the row: it starts at the region's first column rounded
+    // down to 16 bytes and is 16 bytes wider than the region; the columns sit `shift` elements into each row.
+    float *STG = jb_smem;                                                               // [PF+1][3][SUB]
+    float (*RHO)[PP] = reinterpret_cast<float (*)[PP]>(jb_smem + (PF + 1) * 3 * SUB);   // [2][PP]
+    float (*SP)[2][PP] = reinterpret_cast<float (*)[2][PP]>(jb_smem + (PF + 1) * 3 * SUB + 2 * PP);     // [NS][2][PP]
+    uint64_t *full = reinterpret_cast<uint64_t *>(jb_smem + (PF + 1) * 3 * SUB + (2 + 2 * NS) * PP);
     constexpr bool ASYNC = true;   // 2-byte storage: cp.async copies the aligned 4-byte word holding the element
 
     const int rx = threadIdx.x & 31, ry0 = threadIdx.x >> 5;
@@ -100,6 +137,18 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     const int gi_lo = blockIdx.x * OT - NS, gj_lo = blockIdx.y * OT - NS;
     const bool cta_edge = (!per_x && (gi_lo <= 0 || gi_lo + R >= g.nx)) || (!per_y && (gj_lo <= 0 || gj_lo + R >= g.ny));
 
+    const bool tma_cta = use_tma && gi_lo >= 0 && gi_lo + R <= g.nx && gj_lo >= 0 && gj_lo + R <= g.ny;
+    constexpr int ALT = 16 / (int)sizeof(T), BWT = R + ALT, BWB = R + 4;    // box widths: T fields / fp32 b
+    const int xcol = g.gx + gi_lo, shT = xcol & (ALT - 1), shB = xcol & 3;
+    auto tma_issue = [&](int p, int stage) {     // one thread: plane p of the three fields -> staging slot
+        float *st = STG + stage * 3 * SUB;
+        const int zr = rho_index(p, g.nz, per_z) + IGR_NG, zm = map_index(p, g.nz, g.bc[4]) + IGR_NG;
+        jb_mbar_expect_tx(&full[stage], R * (2 * BWT * (int)sizeof(T) + BWB * 4));
+        jb_tma_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo, zr, &full[stage]);
+        jb_tma_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo, zm, &full[stage]);
+        jb_tma_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
+    };
+
     Coef C[CPT][NS];                         // ring: coefficient set of plane p lives in slot p mod NS
     float below[CPT][NS], centre[CPT][NS];   // own column: level-l iterate at planes c-1, c (c = p1 - l)
     float rho1[CPT], b1[CPT], wz_prev[CPT], rn0[CPT], bn0[CPT], sn0[CPT];
@@ -135,14 +184,14 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     auto stage_plane = [&](int p, int stage) {   // asynchronous copy of plane p into a staging slot
         const unsigned zr = usz * (unsigned)(rho_index(p, g.nz, per_z) + IGR_NG);
         const unsigned zm = usz * (unsigned)(map_index(p, g.nz, g.bc[4]) + IGR_NG);
-        float *st = STG + stage * 3 * R * R + threadIdx.x;
+        float *st = STG + stage * 3 * SUB + threadIdx.x;
 #pragma unroll
         for (int cc = 0; cc < CPT; ++cc) {
             // (for 2-byte T the source address is rounded down to its 4-byte word)
             constexpr uintptr_t WORD = (sizeof(T) == 4) ? ~(uintptr_t)0 : ~(uintptr_t)3;
             cp4(st + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(rho + (off_r[cc] + zr)) & WORD));
-            cp4(st + R * R + cc * NTHREADS, bsrc + (off_m[cc] + zm));
-            cp4(st + 2 * R * R + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(sin + (off_m[cc] + zm)) & WORD));
+            cp4(st + SUB + cc * NTHREADS, bsrc + (off_m[cc] + zm));
+            cp4(st + 2 * SUB + cc * NTHREADS, reinterpret_cast<const void *>(reinterpret_cast<uintptr_t>(sin + (off_m[cc] + zm)) & WORD));
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -150,7 +199,14 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
     const int kfirst = kz0 - NS;             // first plane that enters; plane p <-> step p - kfirst
     const int nsteps = nkz + 2 * NS;         // output plane of step tau is kfirst + tau - NS
     const float k22 = 2.0f * k2;
-    if (ASYNC) {
+    if (tma_cta) {
+        if (threadIdx.x == 0) {
+            for (int d = 0; d <= PF; ++d) jb_mbar_init(&full[d], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            for (int d = 0; d < PF; ++d) tma_issue(kfirst + d, d);     // nsteps > PF always
+        }
+    } else if (ASYNC) {
 #pragma unroll
         for (int d = 0; d < PF; ++d) stage_plane(kfirst + d, d);
     } else {
@@ -176,21 +232,38 @@ k_jacobi_blocked(Grid g, const T *__restrict__ rho, const float *__restrict__ bs
             const int tau = base + u;
             const int p0 = kfirst + tau, p1 = p0 - 1;
             float rho0[CPT], b0[CPT], s0[CPT];
-            if (ASYNC) {
+            if (tma_cta) {
+                // the slot of plane p0 + PF was read in the previous step (barrier since): refill it
+                if (threadIdx.x == 0 && tau + PF < nsteps) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    tma_issue(p0 + PF, (tau + PF) % (PF + 1));
+                }
+                // (the last group may run a few steps past nsteps: nothing was loaded for them, their
+                // values are never stored)
+                if (tau < nsteps) jb_mbar_wait(&full[tau % (PF + 1)], (unsigned)(tau / (PF + 1)) & 1u);
+                const float *st = STG + (tau % (PF + 1)) * 3 * SUB;
+#pragma unroll
+                for (int cc = 0; cc < CPT; ++cc) {
+                    const int ry = ry0 + cc * (R / CPT);
+                    b0[cc] = st[SUB + ry * BWB + shB + rx];
+                    rho0[cc] = ldf(reinterpret_cast<const T *>(st) + (ry * BWT + shT + rx));
+                    s0[cc] = ldf(reinterpret_cast<const T *>(st + 2 * SUB) + (ry * BWT + shT + rx));
+                }
+            } else if (ASYNC) {
                 // plane p0 was committed PF steps ago; keep PF groups in flight (empty groups at the end)
                 stage_plane(p0 + PF, (tau + PF) % (PF + 1));
                 asm volatile("cp.async.wait_group %0;" ::"n"(PF) : "memory");
-                const float *st = STG + (tau % (PF + 1)) * 3 * R * R + threadIdx.x;
+                const float *st = STG + (tau % (PF + 1)) * 3 * SUB + threadIdx.x;
 #pragma unroll
                 for (int cc = 0; cc < CPT; ++cc) {
-                    b0[cc] = st[R * R + cc * NTHREADS];
+                    b0[cc] = st[SUB + cc * NTHREADS];
                     if (sizeof(T) == 4) {
-                        rho0[cc] = st[cc * NTHREADS]; s0[cc] = st[2 * R * R + cc * NTHREADS];
+                        rho0[cc] = st[cc * NTHREADS]; s0[cc] = st[2 * SUB + cc * NTHREADS];
                     } else {
                         // pick the element out of its word: the parity of the element offset is the
                         // same for every plane when the plane stride is even (it is: px is a multiple of 16)
                         const T *wr = reinterpret_cast<const T *>(st + cc * NTHREADS);
-                        const T *ws = reinterpret_cast<const T *>(st + 2 * R * R + cc * NTHREADS);
+                        const T *ws = reinterpret_cast<const T *>(st + 2 * SUB + cc * NTHREADS);
                         rho0[cc] = ldf(wr + (off_r[cc] & 1u)); s0[cc] = ldf(ws + (off_m[cc] & 1u));
                     }
                 }
@@ -309,24 +382,80 @@ int jacobi_blocked_zc(const Grid &g, int ns)
     return zc;
 }
 
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 3-D map (x, y, z) of one padded field; box = region + 16 bytes in x (the box start is rounded down to 16 B)
+bool encode_plane_map(CUtensorMap *out, const Grid &g, const void *base, int storage)
+{
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    const size_t es = storage == 0 ? 4 : 2;
+    const CUtensorMapDataType dt = storage == 0 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                   : (storage == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
+    cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz };
+    cuuint64_t strides[2] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es };
+    cuuint32_t box[3] = { (cuuint32_t)(R + 16 / es), R, 1 }, estr[3] = { 1, 1, 1 };   // 16 bytes wider than the region
+    return enc(out, dt, 3, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
+                     const float *b, JacobiMaps *out)
+{
+    out->valid = false;
+    for (int i = 0; i < 3; ++i)
+        if (!encode_plane_map(&out->rho[i], g, st[i < n_state ? i : n_state - 1].f[0], storage)) return 1;
+    for (int i = 0; i < 2; ++i)
+        if (!encode_plane_map(&out->sig[i], g, sig[i], storage)) return 1;
+    if (!encode_plane_map(&out->b, g, b, 0)) return 1;
+    out->valid = true;
+    return 0;
+}
+
 template <typename T>
 static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, const void *sin, void *sout,
-                      float k2, cudaStream_t st)
+                      float k2, const CUtensorMap *rmap, const CUtensorMap *bmap, const CUtensorMap *smap,
+                      cudaStream_t st)
 {
     const int ot = R - 2 * ns, zc = jacobi_blocked_zc(g, ns);
     dim3 grid((g.nx + ot - 1) / ot, (g.ny + ot - 1) / ot, (g.nz + zc - 1) / zc);
-    const int smem = (2 + 2 * ns) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4;
+    const int use_tma = (rmap && bmap && smap) ? 1 : 0;
+    static const CUtensorMap dummy = {};
+    const CUtensorMap &rm = use_tma ? *rmap : dummy, &bm = use_tma ? *bmap : dummy, &sm = use_tma ? *smap : dummy;
+#define IGR_JB_SMEM(NSV) ((2 + 2 * (NSV)) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * SUB * 4 + (PF + 1) * 8 + 8)
+    const int smem = IGR_JB_SMEM(ns);
 #define IGR_JB(NSV)                                                                                      \
     do {                                                                                                 \
         constexpr int CPTV = (NSV <= 3) ? cpt_small : 2;                                                 \
         static bool configured = false;                                                                  \
         if (!configured) {                                                                               \
             cudaFuncSetAttribute(k_jacobi_blocked<T, NSV, CPTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                 (2 + 2 * NSV) * (R + 2) * (R + 2) * 4 + (PF + 1) * 3 * R * R * 4);      \
+                                 IGR_JB_SMEM(NSV));                                                      \
             configured = true;                                                                           \
         }                                                                                                \
-        k_jacobi_blocked<T, NSV, CPTV><<<grid, R * R / CPTV, smem, st>>>(g, (const T *)rho, b, (const T *)sin, \
-                                                                    (T *)sout, k2, zc);                 \
+        k_jacobi_blocked<T, NSV, CPTV><<<grid, R * R / CPTV, smem, st>>>(rm, bm, sm, use_tma, g, (const T *)rho, b, \
+                                                                    (const T *)sin, (T *)sout, k2, zc);  \
     } while (0)
     switch (ns) {
     case 1: IGR_JB(1); break;
@@ -336,13 +465,16 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
     default: IGR_JB(5); break;
     }
 #undef IGR_JB
+#undef IGR_JB_SMEM
 }
 
-// ns in 1..5 sweeps in one pass; sig_in and sig_out must differ
+// ns in 1..5 sweeps in one pass; sig_in and sig_out must differ.  With the three maps (planes of rho, b and
+// sig_in) regions inside the domain stage their planes by TMA; NULL maps: cp.async everywhere.
 void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, const float *b,
-                           const void *sig_in, void *sig_out, float k2, cudaStream_t st)
+                           const void *sig_in, void *sig_out, float k2, const CUtensorMap *rmap,
+                           const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st)
 {
-    if (storage == 0) launch_ns<float>(g, ns, rho, b, sig_in, sig_out, k2, st);
-    else if (storage == 1) launch_ns<__half>(g, ns, rho, b, sig_in, sig_out, k2, st);
-    else launch_ns<__nv_bfloat16>(g, ns, rho, b, sig_in, sig_out, k2, st);
+    if (storage == 0) launch_ns<float>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
+    else if (storage == 1) launch_ns<__half>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
+    else launch_ns<__nv_bfloat16>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
 }

@@ -2,6 +2,7 @@
 // SURVEY.md 8(a)).  `storage` is IGR_STORE_F32 / F16 / BF16 (igr.h); q and Sigma use that element
 // type, b and r are always fp32.
 #pragma once
+#include <cuda.h>
 #include "igr_common.cuh"
 
 struct RhsParams {
@@ -53,6 +54,15 @@ void launch_rk_update(const Grid &g, int storage, StagePtrs qn, StagePtrs qs, St
 void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, WaveResult *wave,
                       cudaStream_t st);
 
-// a3 (blocked form): ns in 1..5 sweeps in ONE pass over HBM (igr_jacobi_blocked.cu); sig_in != sig_out
+// a3 (blocked form): ns in 1..5 sweeps in ONE pass over HBM (igr_jacobi_blocked.cu); sig_in != sig_out.
+// TMA maps of the planes of rho (the three state buffers), Sigma (two buffers) and b: regions inside the
+// domain stage their planes with them; NULL maps: every region gathers with cp.async.
+struct JacobiMaps {
+    CUtensorMap rho[3], sig[2], b;
+    bool valid;
+};
+int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
+                     const float *b, JacobiMaps *out);
 void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, const float *b,
-                           const void *sig_in, void *sig_out, float k2, cudaStream_t st);
+                           const void *sig_in, void *sig_out, float k2, const CUtensorMap *rmap,
+                           const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st);
