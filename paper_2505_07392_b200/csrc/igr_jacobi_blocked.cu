@@ -31,6 +31,18 @@ __device__ __forceinline__ void jb_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(jb_smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void jb_mbar_wait_s32(uint32_t bar, uint32_t parity)    // bar: shared-window address
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "JB_WAIT2:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra JB_DONE2;\n"
+        "bra JB_WAIT2;\n"
+        "JB_DONE2:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void jb_mbar_wait(uint64_t *bar, uint32_t parity)
 {
     asm volatile(
@@ -149,6 +161,10 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
         jb_tma_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
     };
 
+    static_assert(PF == 3, "slot arithmetic assumes a ring of 4");
+    const uint32_t full_s = jb_smem_u32(full);
+    unsigned slot = 0, phase = 0;            // staging slot of the plane consumed in this step, its phase
+
     Coef C[CPT][NS];                         // ring: coefficient set of plane p lives in slot p mod NS
     float below[CPT][NS], centre[CPT][NS];   // own column: level-l iterate at planes c-1, c (c = p1 - l)
     float rho1[CPT], b1[CPT], wz_prev[CPT], rn0[CPT], bn0[CPT], sn0[CPT];
@@ -236,12 +252,13 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
                 // the slot of plane p0 + PF was read in the previous step (barrier since): refill it
                 if (threadIdx.x == 0 && tau + PF < nsteps) {
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    tma_issue(p0 + PF, (tau + PF) % (PF + 1));
+                    tma_issue(p0 + PF, (slot + PF) & PF);          // (slot + PF) mod (PF + 1), PF + 1 = 4
                 }
                 // (the last group may run a few steps past nsteps: nothing was loaded for them, their
                 // values are never stored)
-                if (tau < nsteps) jb_mbar_wait(&full[tau % (PF + 1)], (unsigned)(tau / (PF + 1)) & 1u);
-                const float *st = STG + (tau % (PF + 1)) * 3 * SUB;
+                if (tau < nsteps) jb_mbar_wait_s32(full_s + 8u * slot, phase);
+                const float *st = STG + slot * (3 * SUB);
+                if (++slot == PF + 1) { slot = 0; phase ^= 1u; }
 #pragma unroll
                 for (int cc = 0; cc < CPT; ++cc) {
                     const int ry = ry0 + cc * (R / CPT);
