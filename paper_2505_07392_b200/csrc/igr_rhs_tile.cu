@@ -3,7 +3,7 @@
 //
 // Design: 2.5-D streaming.  A CTA owns a 32 x TY column of cells and marches
 // along z.  Whole xy-planes of the six fields (q[5] as one 4-D box, Sigma as a 3-D box) with their
-// 3-cell halos are staged into a 6-slot shared-memory ring by TMA (cp.async.bulk.tensor + mbarrier),
+// 3-cell halos are staged into a 7-slot shared-memory ring by TMA (cp.async.bulk.tensor + mbarrier),
 // three planes ahead of use.  Each thread owns one (x, y) column: the z stencil lives in a sliding
 // register window (6 planes x 6 fields), the x and y stencils are read from the current plane in
 // shared memory.  Every face flux is computed exactly once per CTA: a thread computes the right (x+),
@@ -25,7 +25,7 @@
 namespace {
 
 constexpr int TX = 32;          // tile width = warp width
-constexpr int NSLOT = 6;        // ring slots (planes): 4 live + 2 in flight
+constexpr int NSLOT = 7;        // ring slots (planes): 4 live + 3 in flight
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -221,7 +221,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        for (int p = 0; p < NSLOT; ++p) issue(p, p);               // n_planes >= 7 > NSLOT
+        for (int p = 0; p < NSLOT; ++p) issue(p, p);               // n_planes >= 7 >= NSLOT
     }
     __syncthreads();
 
@@ -308,9 +308,11 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 
     float vmax = 0.f;
     bool bad = false;
+    // element offsets fit 32 bits (unsigned) on any grid that fits the device
+    unsigned uid = (unsigned)(i + g.gx) + (unsigned)g.sy * (unsigned)(j + IGR_NG) + (unsigned)g.sz * (unsigned)(kz0 + IGR_NG);
 
     // ---- march: step t computes cell plane k = kz0 + t; current plane p = t + 3
-    int slot_c = 3, slot_n = 0, phase_n = 1;                      // slots of planes t + 3 and t + 6
+    int slot_c = 3, slot_n = 6 % NSLOT, phase_n = (6 / NSLOT) & 1;  // slots of planes t + 3 and t + 6
     for (int t = 0; t < nkz; ++t) {
         const int pc = t + 3;
         const int slot_c1 = (slot_c == NSLOT - 1) ? 0 : slot_c + 1;  // slot of plane pc + 1
@@ -324,7 +326,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         // fused update: q^n of this cell is fetched now and consumed at the end of the step, so that
         // the global-load latency hides behind the flux computation
         float qn_pre[5];
-        const long long id = g.idx(i, j, kz0 + t);
+        const unsigned id = uid;                                    // element offset of cell (i, j, kz0 + t)
+        uid += (unsigned)g.sz;
         if (FUSE) {
 #pragma unroll
             for (int c = 0; c < 5; ++c)
@@ -401,9 +404,9 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
         }
         __syncthreads();                                   // the only barrier of the step
-        if (tid == 0 && t + 9 < n_planes) {                      // slot of plane pc is free again
+        if (tid == 0 && t + 3 + NSLOT < n_planes) {              // slot of plane pc is free again
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            issue(t + 9, slot_c);
+            issue(t + 3 + NSLOT, slot_c);
         }
 
         // z+ face (cells k-2 .. k+3 of the own column), then the divergence
