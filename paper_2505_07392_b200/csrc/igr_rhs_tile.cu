@@ -309,7 +309,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     float vmax = 0.f;
     bool bad = false;
     // element offsets fit 32 bits (unsigned) on any grid that fits the device
-    unsigned uid = (unsigned)(i + g.gx) + (unsigned)g.sy * (unsigned)(j + IGR_NG) + (unsigned)g.sz * (unsigned)(kz0 + IGR_NG);
+    unsigned uid = (unsigned)(min(i, g.nx - 1) + g.gx) + (unsigned)g.sy * (unsigned)(min(j, g.ny - 1) + IGR_NG) +
+                   (unsigned)g.sz * (unsigned)(kz0 + IGR_NG);
 
     // ---- march: step t computes cell plane k = kz0 + t; current plane p = t + 3
     int slot_c = 3, slot_n = 6 % NSLOT, phase_n = (6 / NSLOT) & 1;  // slots of planes t + 3 and t + 6
@@ -328,10 +329,9 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         float qn_pre[5];
         const unsigned id = uid;                                    // element offset of cell (i, j, kz0 + t)
         uid += (unsigned)g.sz;
-        if (FUSE) {
-#pragma unroll
-            for (int c = 0; c < 5; ++c)
-                qn_pre[c] = (a.read_qn && valid) ? ldf(reinterpret_cast<const T *>(a.qn[c]) + id) : 0.f;
+        if (FUSE && a.read_qn) {                                   // (columns beyond the domain read a valid
+#pragma unroll                                                      //  cell: the offset is clamped, nothing is stored)
+            for (int c = 0; c < 5; ++c) qn_pre[c] = ldf(reinterpret_cast<const T *>(a.qn[c]) + id);
         }
         // wave speeds of the next cell (k+1) of this column, published for the next step
         float ax_n, ay_n, az_n;
