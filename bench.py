@@ -155,7 +155,7 @@ def alg_bytes(row, storage, fused=1):
 ALG_FLOP = {"sigma_source": 45.0, "jacobi": 90.0, "rhs": 614.0, "rk_update": 20.0}
 # DRAM bytes per cell per launch measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum,
 # profiles/r01_ncu_full_*): fp32 storage, stage-1 launch of the fused RHS kernel
-NCU_DRAM_BYTES_PER_CELL = {"f32": {"sigma_source": 20.8, "jacobi": 21.3, "rhs": 47.6}}
+NCU_DRAM_BYTES_PER_CELL = {"f32": {"sigma_source": 21.2, "jacobi": 21.4, "rhs": 47.6}}
 
 
 def alu_peak_tflops():
