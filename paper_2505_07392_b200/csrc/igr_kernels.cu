@@ -267,9 +267,10 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
     struct Raw { float r[4], h[4]; };
     auto fetch = [&](int k, Raw &w) {
         const unsigned zo = usz * (unsigned)(min(k, g.nz) + IGR_NG);
-        w.r[0] = ldf(rho + col + zo); w.r[1] = ldf(m[0] + col + zo); w.r[2] = ldf(m[1] + col + zo); w.r[3] = ldf(m[2] + col + zo);
+        const unsigned o = col + zo, ho = hcol + zo;              // one 32-bit offset for the four fields
+        w.r[0] = ldf(rho + o); w.r[1] = ldf(m[0] + o); w.r[2] = ldf(m[1] + o); w.r[3] = ldf(m[2] + o);
         if (hpos >= 0) {
-            w.h[0] = ldf(rho + hcol + zo); w.h[1] = ldf(m[0] + hcol + zo); w.h[2] = ldf(m[1] + hcol + zo); w.h[3] = ldf(m[2] + hcol + zo);
+            w.h[0] = ldf(rho + ho); w.h[1] = ldf(m[0] + ho); w.h[2] = ldf(m[1] + ho); w.h[3] = ldf(m[2] + ho);
         }
     };
     auto put_plane = [&](int buf, const Raw &w, float v[3]) {               // fetched plane -> velocities
