@@ -104,6 +104,7 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
     // own column in global memory (columns beyond the domain are clamped into the padding: unused values)
     const unsigned col = (unsigned)(min(i, g.nx) + g.gx) + (unsigned)g.sy * (unsigned)(min(j, g.ny) + IGR_NG);
     const unsigned usz = (unsigned)g.sz;
+    const unsigned colc = (unsigned)(min(i, g.nx - 1) + g.gx) + (unsigned)g.sy * (unsigned)(min(j, g.ny - 1) + IGR_NG);
     const T *qf[4] = { (const T *)a.q[0], (const T *)a.q[1], (const T *)a.q[2], (const T *)a.q[3] };
     const float *tz[3] = { a.tau + (size_t)IGR_TAU_XZ * g.np, a.tau + (size_t)IGR_TAU_YZ * g.np,
                            a.tau + (size_t)IGR_TAU_ZZ * g.np };
@@ -145,17 +146,18 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
 #pragma unroll
         for (int f = 0; f < 7; ++f) W[f][5] = pre[f];
         fetch(kz0 + t + 4, pre);                                   // lands during this step
-        const long long id = g.idx(min(i, g.nx), min(j, g.ny), kz0 + t);
+        const unsigned id = colc + usz * (unsigned)(kz0 + t + IGR_NG);   // clamped column: reads are always valid
         float r_pre[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) r_pre[c] = valid ? a.r[1 + c][id] : 0.f;
+        for (int c = 0; c < 4; ++c) r_pre[c] = a.r[1 + c][id];
         // fused update: everything the epilogue reads pointwise is fetched now
         float r0 = 0.f, Es = 0.f, qn_pre[5];
         if (FUSE) {
-            if (valid) { r0 = a.r[0][id]; Es = ldf(reinterpret_cast<const T *>(a.q[4]) + id); }
+            r0 = a.r[0][id]; Es = ldf(reinterpret_cast<const T *>(a.q[4]) + id);
+            if (a.read_qn) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c)
-                qn_pre[c] = (a.read_qn && valid) ? ldf(reinterpret_cast<const T *>(a.qn[c]) + id) : 0.f;
+                for (int c = 0; c < 5; ++c) qn_pre[c] = ldf(reinterpret_cast<const T *>(a.qn[c]) + id);
+            }
         }
 
         mbar_wait(&full[slot], phase);
