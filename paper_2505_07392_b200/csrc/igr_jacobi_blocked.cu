@@ -15,51 +15,13 @@
 // periodic directions are recomputed from wrapped data, clamp directions read the cell itself in
 // place of its outside neighbour.
 #include "igr_kernels.h"
+#include "igr_tma.cuh"
 
 #include <cuda.h>
 #include <cstdlib>
 #include <type_traits>
 
 namespace {
-
-__device__ __forceinline__ uint32_t jb_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void jb_mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(jb_smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void jb_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(jb_smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void jb_mbar_wait_s32(uint32_t bar, uint32_t parity)    // bar: shared-window address
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "JB_WAIT2:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra JB_DONE2;\n"
-        "bra JB_WAIT2;\n"
-        "JB_DONE2:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void jb_mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "JB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra JB_DONE;\n"
-        "bra JB_WAIT;\n"
-        "JB_DONE:\n"
-        "}\n" ::"r"(jb_smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void jb_tma_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(jb_smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(jb_smem_u32(bar)) : "memory");
-}
 
 constexpr int R = 32;                       // region edge
 constexpr int cpt_small = 2;                // columns per thread for NS <= 3 (1 = 1024 threads: measured slower)
@@ -155,14 +117,14 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
     auto tma_issue = [&](int p, int stage) {     // one thread: plane p of the three fields -> staging slot
         float *st = STG + stage * 3 * SUB;
         const int zr = rho_index(p, g.nz, per_z) + IGR_NG, zm = map_index(p, g.nz, g.bc[4]) + IGR_NG;
-        jb_mbar_expect_tx(&full[stage], R * (2 * BWT * (int)sizeof(T) + BWB * 4));
-        jb_tma_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo, zr, &full[stage]);
-        jb_tma_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo, zm, &full[stage]);
-        jb_tma_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
+        igr_tma::mbar_expect_tx(&full[stage], R * (2 * BWT * (int)sizeof(T) + BWB * 4));
+        igr_tma::tma_load_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo, zr, &full[stage]);
+        igr_tma::tma_load_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo, zm, &full[stage]);
+        igr_tma::tma_load_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
     };
 
     static_assert(PF == 3, "slot arithmetic assumes a ring of 4");
-    const uint32_t full_s = jb_smem_u32(full);
+    const uint32_t full_s = igr_tma::smem_u32(full);
     unsigned slot = 0, phase = 0;            // staging slot of the plane consumed in this step, its phase
 
     Coef C[CPT][NS];                         // ring: coefficient set of plane p lives in slot p mod NS
@@ -217,9 +179,8 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
     const float k22 = 2.0f * k2;
     if (tma_cta) {
         if (threadIdx.x == 0) {
-            for (int d = 0; d <= PF; ++d) jb_mbar_init(&full[d], 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            for (int d = 0; d <= PF; ++d) igr_tma::mbar_init(&full[d], 1);
+            igr_tma::fence_init();
             for (int d = 0; d < PF; ++d) tma_issue(kfirst + d, d);     // nsteps > PF always
         }
     } else if (ASYNC) {
@@ -251,12 +212,12 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
             if (tma_cta) {
                 // the slot of plane p0 + PF was read in the previous step (barrier since): refill it
                 if (threadIdx.x == 0 && tau + PF < nsteps) {
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    igr_tma::fence_async();
                     tma_issue(p0 + PF, (slot + PF) & PF);          // (slot + PF) mod (PF + 1), PF + 1 = 4
                 }
                 // (the last group may run a few steps past nsteps: nothing was loaded for them, their
                 // values are never stored)
-                if (tau < nsteps) jb_mbar_wait_s32(full_s + 8u * slot, phase);
+                if (tau < nsteps) igr_tma::mbar_wait_s32(full_s + 8u * slot, phase);
                 const float *st = STG + slot * (3 * SUB);
                 if (++slot == PF + 1) { slot = 0; phase ^= 1u; }
 #pragma unroll
@@ -401,38 +362,14 @@ int jacobi_blocked_zc(const Grid &g, int ns)
 
 namespace {
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
 // 3-D map (x, y, z) of one padded field; box = region + 16 bytes in x (the box start is rounded down to 16 B)
 bool encode_plane_map(CUtensorMap *out, const Grid &g, const void *base, int storage)
 {
-    EncodeTiledFn enc = get_encode();
-    if (!enc) return false;
     const size_t es = storage == 0 ? 4 : 2;
-    const CUtensorMapDataType dt = storage == 0 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
-                                   : (storage == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
     cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz };
     cuuint64_t strides[2] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es };
-    cuuint32_t box[3] = { (cuuint32_t)(R + 16 / es), R, 1 }, estr[3] = { 1, 1, 1 };   // 16 bytes wider than the region
-    return enc(out, dt, 3, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    cuuint32_t box[3] = { (cuuint32_t)(R + 16 / es), R, 1 };     // 16 bytes wider than the region
+    return igr_tma::encode(out, igr_tma::data_type(storage), 3, base, dims, strides, box);
 }
 
 }  // namespace

@@ -15,6 +15,7 @@
 //
 // Arithmetic (same as k_rhs_simple): Alg. 1, eqs. 6-8 L119-L125.
 #include "igr_rhs_tile.cuh"
+#include "igr_tma.cuh"
 
 #include <cstdio>
 #include <type_traits>
@@ -27,38 +28,8 @@ namespace {
 constexpr int TX = 32;          // tile width = warp width
 constexpr int NSLOT = 7;        // ring slots (planes): 4 live + 3 in flight
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+using namespace igr_tma;
 
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ float rcp_fast(float x)
 {
     float y;
@@ -219,8 +190,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     const int n_planes = nkz + 6;                                  // planes kz0-3 .. kz0+nkz+2
     if (tid == 0) {
         for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_init();
         for (int p = 0; p < NSLOT; ++p) issue(p, p);               // n_planes >= 7 >= NSLOT
     }
     __syncthreads();
@@ -302,7 +272,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     put_speeds(3, 3, ax_c, ay_c);                                  // plane of the first cell layer kz0
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_async();
         for (int p = NSLOT; p < NSLOT + 3 && p < n_planes; ++p) issue(p, p - NSLOT);
     }
 
@@ -405,7 +375,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         }
         __syncthreads();                                   // the only barrier of the step
         if (tid == 0 && t + 3 + NSLOT < n_planes) {              // slot of plane pc is free again
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            fence_async();
             issue(t + 3 + NSLOT, slot_c);
         }
 
@@ -472,24 +442,6 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 // ======================================================================================= host
 namespace {
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
 int tile_ty(const Grid &g)
 {
     static int force = -1;                       // IGR_RHS_TY=8|16 overrides the heuristic (tuning)
@@ -518,11 +470,9 @@ int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_
                        RhsTileMaps *out, const char **err)
 {
     out->valid = false;
-    EncodeTiledFn enc = get_encode();
-    if (!enc) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
+    if (!igr_tma::get_encode()) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
     const size_t es = storage == 0 ? 4 : 2;
-    const CUtensorMapDataType dt = storage == 0 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
-                                   : (storage == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
+    const CUtensorMapDataType dt = igr_tma::data_type(storage);
     const int hx = 16 / (int)es, ty = tile_ty(g);
     const cuuint32_t bx = TX + 2 * hx, by = ty + 6;
     for (int b = 0; b < 3; ++b) {
@@ -530,20 +480,14 @@ int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_
         const cuuint64_t fstride = (cuuint64_t)((char *)s.f[1] - (char *)s.f[0]);
         cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 5 };
         cuuint64_t strides[3] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es, fstride };
-        cuuint32_t box[4] = { bx, by, 1, 5 }, estr[4] = { 1, 1, 1, 1 };
-        CUresult rc = enc(&out->q[b], dt, 4, s.f[0], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(q) failed"; return (int)rc; }
+        cuuint32_t box[4] = { bx, by, 1, 5 };
+        if (!igr_tma::encode(&out->q[b], dt, 4, s.f[0], dims, strides, box)) { *err = "cuTensorMapEncodeTiled(q) failed"; return 2; }
     }
     for (int b = 0; b < 2; ++b) {
         cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz };
         cuuint64_t strides[2] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es };
-        cuuint32_t box[3] = { bx, by, 1 }, estr[3] = { 1, 1, 1 };
-        CUresult rc = enc(&out->sig[b], dt, 3, sig[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(sigma) failed"; return (int)rc; }
+        cuuint32_t box[3] = { bx, by, 1 };
+        if (!igr_tma::encode(&out->sig[b], dt, 3, sig[b], dims, strides, box)) { *err = "cuTensorMapEncodeTiled(sigma) failed"; return 2; }
     }
     out->valid = true;
     return 0;

@@ -9,6 +9,7 @@
 // x- by shuffle, y- through shared memory, z- from the previous step; the low-x and low-y tile edges by
 // two designated warps.  One __syncthreads per plane (exchange buffers double-buffered by step parity).
 #include "igr_viscous.cuh"
+#include "igr_tma.cuh"
 
 #include <type_traits>
 
@@ -17,32 +18,7 @@ namespace {
 constexpr int TX = 32, TY = 8, NT = TX * TY;
 constexpr int NSLOT = 3;
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "VLAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra VDONE;\n"
-        "bra VLAB_WAIT;\n"
-        "VDONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
-}
+using namespace igr_tma;
 
 template <typename T>
 struct VTile {
@@ -95,8 +71,7 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
     };
     if (tid == 0) {
         for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_init();
         for (int p = 0; p < NSLOT && p < nkz; ++p) issue(p, p);
     }
     __syncthreads();
@@ -234,7 +209,7 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
         }
         __syncthreads();                                    // the only barrier of the step
         if (tid == 0 && t + NSLOT < nkz) {                  // the slot of this plane is free again
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            fence_async();
             issue(t + NSLOT, slot);
         }
 
@@ -291,24 +266,6 @@ k_viscous_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__
 // ======================================================================================= host
 namespace {
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode()
-{
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
 template <typename T, int ORDER, bool FUSE>
 void launch_one(const Grid &g, const CUtensorMap &qmap, const CUtensorMap &tmap, ViscTileArgs a, cudaStream_t st)
 {
@@ -328,13 +285,9 @@ int visc_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n
                         ViscTileMaps *out, const char **err)
 {
     out->valid = false;
-    EncodeTiledFn enc = get_encode();
-    if (!enc) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
+    if (!igr_tma::get_encode()) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
     const size_t es = storage == 0 ? 4 : 2;
-    const CUtensorMapDataType dt = storage == 0 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
-                                   : (storage == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
     const cuuint32_t bx = TX + 2 * (16 / (cuuint32_t)es), by = TY + 6;
-    cuuint32_t estr[4] = { 1, 1, 1, 1 };
     for (int b = 0; b < 3; ++b) {
         const StagePtrs &s = st[b < n_state ? b : n_state - 1];
         const cuuint64_t fstride = (cuuint64_t)((char *)s.f[1] - (char *)s.f[0]);
@@ -345,19 +298,17 @@ int visc_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n
         cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 4 };
         cuuint64_t strides[3] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es, fstride };
         cuuint32_t box[4] = { bx, by, 1, 4 };
-        CUresult rc = enc(&out->q[b], dt, 4, s.f[0], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(q, viscous) failed"; return (int)rc; }
+        if (!igr_tma::encode(&out->q[b], igr_tma::data_type(storage), 4, s.f[0], dims, strides, box)) {
+            *err = "cuTensorMapEncodeTiled(q, viscous) failed"; return 3;
+        }
     }
     {
         cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 5 };
         cuuint64_t strides[3] = { (cuuint64_t)g.px * 4, (cuuint64_t)g.px * g.py * 4, (cuuint64_t)g.np * 4 };
         cuuint32_t box[4] = { TX + 8, by, 1, 5 };
-        CUresult rc = enc(&out->tau, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)tau, dims, strides, box, estr,
-                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (rc != CUDA_SUCCESS) { *err = "cuTensorMapEncodeTiled(tau) failed"; return (int)rc; }
+        if (!igr_tma::encode(&out->tau, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, tau, dims, strides, box)) {
+            *err = "cuTensorMapEncodeTiled(tau) failed"; return 3;
+        }
     }
     out->valid = true;
     return 0;
