@@ -318,21 +318,30 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
     fetch(kz0, A);
     int bc = 0;                                              // buffer of plane k (k = kz0 + t), mod NB
     put_plane(bc, A, ce);
+    // planes per barrier: two with 4-byte storage (4.94 -> 4.72 ms at 1024^3), one with 2-byte storage (two
+    // measured slower there: 7.1 vs 5.2 ms)
+    constexpr int PPB = (sizeof(T) == 4) ? 2 : 1;
     fetch(kz0 + 1, A);
-    fetch(kz0 + 2, B);
-    for (int t = 0; t < nkz; t += 2) {
+    if (PPB == 2) fetch(kz0 + 2, B);
+    for (int t = 0; t < nkz; t += PPB) {
         const int k = kz0 + t;
         const int b1 = (bc + 1 >= NB) ? bc + 1 - NB : bc + 1, b2 = (bc + 2 >= NB) ? bc + 2 - NB : bc + 2;
         put_plane(b1, A, u1);                                // plane k + 1
-        put_plane(b2, B, u2);                                // plane k + 2 (ghost plane at the top)
-        fetch(k + 3, A);                                     // land during this iteration
-        fetch(k + 4, B);
-        __syncthreads();                                     // one barrier per two planes
+        if (PPB == 2) put_plane(b2, B, u2);                  // plane k + 2 (ghost plane at the top)
+        fetch(k + 1 + PPB, A);                               // land during this iteration
+        if (PPB == 2) fetch(k + 2 + PPB, B);
+        __syncthreads();                                     // one barrier per PPB planes
         emit(k, U[bc], dn, u1);
-        if (t + 1 < nkz) emit(k + 1, U[b1], ce, u2);
+        if (PPB == 2) {
+            if (t + 1 < nkz) emit(k + 1, U[b1], ce, u2);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { dn[a] = u1[a]; ce[a] = u2[a]; }
-        bc = b2;
+            for (int a = 0; a < 3; ++a) { dn[a] = u1[a]; ce[a] = u2[a]; }
+            bc = b2;
+        } else {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { dn[a] = ce[a]; ce[a] = u1[a]; }
+            bc = b1;
+        }
     }
 }
 
