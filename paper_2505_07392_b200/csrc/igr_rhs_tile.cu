@@ -26,7 +26,9 @@
 namespace {
 
 constexpr int TX = 32;          // tile width = warp width
-constexpr int NSLOT = 7;        // ring slots (planes): 4 live + 3 in flight
+#ifndef IGR_RHS_NSLOT_HALF
+#define IGR_RHS_NSLOT_HALF 6
+#endif
 
 using namespace igr_tma;
 
@@ -44,8 +46,9 @@ __device__ __forceinline__ float sqrt_fast(float x)
 }
 
 // ---- geometry of one ring slot for storage type T
-template <typename T, int TY>
+template <typename T, int TY, int NSLOT_OF_T = (sizeof(T) == 4 ? 7 : IGR_RHS_NSLOT_HALF)>
 struct Tile {
+    static constexpr int NSLOT = NSLOT_OF_T;             // ring slots (planes): 4 live + 2 or 3 in flight
     static constexpr int HX = 16 / (int)sizeof(T);       // x halo of the box: 4 (fp32) / 8 (half) -> 16 B
     static constexpr int BX = TX + 2 * HX;               // box extents
     static constexpr int BY = TY + 6;
@@ -181,7 +184,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 
     // TMA coordinates of the box origin in the padded arrays (elements)
     const int cx = g.gx + x0 - TL::HX, cy = y0, cz0 = kz0;       // plane p <-> padded z = kz0 + p
-    auto issue = [&](int p, int slot) {                           // one elected thread; slot = p mod NSLOT
+    auto issue = [&](int p, int slot) {                           // one elected thread; slot = p mod TL::NSLOT
         unsigned char *dst = smem + slot * TL::SLOT;
         mbar_expect_tx(&full[slot], TL::TXBYTES);
         tma_load_4d(dst, &qmap, cx, cy, cz0 + p, 0, &full[slot]);
@@ -189,14 +192,14 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     };
     const int n_planes = nkz + 6;                                  // planes kz0-3 .. kz0+nkz+2
     if (tid == 0) {
-        for (int s = 0; s < NSLOT; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < TL::NSLOT; ++s) mbar_init(&full[s], 1);
         fence_init();
-        for (int p = 0; p < NSLOT; ++p) issue(p, p);               // n_planes >= 7 >= NSLOT
+        for (int p = 0; p < TL::NSLOT; ++p) issue(p, p);               // n_planes >= 7 >= TL::NSLOT
     }
     __syncthreads();
 
     const int own = (3 + ty) * TL::BX + TL::HX + tx;               // own cell inside a plane box
-    // slot = plane index mod NSLOT; the march keeps the slot indices as wrapping counters (no division)
+    // slot = plane index mod TL::NSLOT; the march keeps the slot indices as wrapping counters (no division)
     auto qbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT); };
     auto sbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT + TL::QBYTES); };
 
@@ -273,7 +276,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
         fence_async();
-        for (int p = NSLOT; p < NSLOT + 3 && p < n_planes; ++p) issue(p, p - NSLOT);
+        for (int p = TL::NSLOT; p < TL::NSLOT + 3 && p < n_planes; ++p) issue(p, p - TL::NSLOT);
     }
 
     float vmax = 0.f;
@@ -283,10 +286,10 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
                    (unsigned)g.sz * (unsigned)(kz0 + IGR_NG);
 
     // ---- march: step t computes cell plane k = kz0 + t; current plane p = t + 3
-    int slot_c = 3, slot_n = 6 % NSLOT, phase_n = (6 / NSLOT) & 1;  // slots of planes t + 3 and t + 6
+    int slot_c = 3, slot_n = 6 % TL::NSLOT, phase_n = (6 / TL::NSLOT) & 1;  // slots of planes t + 3 and t + 6
     for (int t = 0; t < nkz; ++t) {
         const int pc = t + 3;
-        const int slot_c1 = (slot_c == NSLOT - 1) ? 0 : slot_c + 1;  // slot of plane pc + 1
+        const int slot_c1 = (slot_c == TL::NSLOT - 1) ? 0 : slot_c + 1;  // slot of plane pc + 1
         mbar_wait(&full[slot_n], phase_n);
         {
             const T *qb = qbase(slot_n) + own;
@@ -374,9 +377,9 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
         }
         __syncthreads();                                   // the only barrier of the step
-        if (tid == 0 && t + 3 + NSLOT < n_planes) {              // slot of plane pc is free again
+        if (tid == 0 && t + 3 + TL::NSLOT < n_planes) {              // slot of plane pc is free again
             fence_async();
-            issue(t + 3 + NSLOT, slot_c);
+            issue(t + 3 + TL::NSLOT, slot_c);
         }
 
         // z+ face (cells k-2 .. k+3 of the own column), then the divergence
@@ -425,7 +428,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         }
         ax_c = ax_n; ay_c = ay_n; az_c = az_n;
         slot_c = slot_c1;
-        if (++slot_n == NSLOT) { slot_n = 0; phase_n ^= 1; }
+        if (++slot_n == TL::NSLOT) { slot_n = 0; phase_n ^= 1; }
     }
 
     if (FUSE && a.wave) {
