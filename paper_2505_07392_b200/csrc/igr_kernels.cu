@@ -323,6 +323,8 @@ __global__ void __launch_bounds__(SRC_TX * SRC_TY) k_source(Grid g, StagePtrs q,
     constexpr int PPB = (sizeof(T) == 4) ? 2 : 1;
     fetch(kz0 + 1, A);
     if (PPB == 2) fetch(kz0 + 2, B);
+    constexpr int TRIP = (PPB == 2) ? 1 : 2;               // two planes per loop trip either way
+#pragma unroll TRIP
     for (int t = 0; t < nkz; t += PPB) {
         const int k = kz0 + t;
         const int b1 = (bc + 1 >= NB) ? bc + 1 - NB : bc + 1, b2 = (bc + 2 >= NB) ? bc + 2 - NB : bc + 2;
