@@ -514,14 +514,24 @@ int igr_jacobi(igr_solver *s)
         if (maxns < 0) { const char *e = getenv("IGR_JACOBI_MAXNS"); maxns = e ? atoi(e) : 5; if (maxns < 1 || maxns > 5) maxns = 5; }
         static int no_tma = -1;                  // IGR_JACOBI_TMA=0: cp.async staging everywhere (tuning)
         if (no_tma < 0) { const char *e = getenv("IGR_JACOBI_TMA"); no_tma = (e && atoi(e) == 0) ? 1 : 0; }
+        static int no_quad = -1;                 // IGR_JACOBI_QUAD=0: the blocked kernel in every region (tuning)
+        if (no_quad < 0) { const char *e = getenv("IGR_JACOBI_QUAD"); no_quad = (e && atoi(e) == 0) ? 1 : 0; }
         const int npass = (s->n_jacobi + maxns - 1) / maxns;
-        RowTimer t(s, 2, npass + 1);
+        RowTimer t(s, 2, 2 * npass + 1);
         for (int left = s->n_jacobi; left > 0; left -= maxns) {
             const bool tma = s->jmaps.valid && !no_tma;
-            launch_jacobi_blocked(s->g, s->storage, left < maxns ? left : maxns, s->st[s->cur].f[0], s->b,
+            const int ns = left < maxns ? left : maxns;
+            // regions that need no periodic wrap in x / y: four columns per thread (igr_jacobi_quad.cu);
+            // the blocked kernel keeps the others
+            JacobiQuadPlan quad = {};
+            if (tma && !no_quad) quad = jacobi_quad_plan(s->g, ns, k2);
+            launch_jacobi_blocked(s->g, s->storage, ns, s->st[s->cur].f[0], s->b,
                                   s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2,
                                   tma ? &s->jmaps.rho[s->cur] : nullptr, tma ? &s->jmaps.b : nullptr,
-                                  tma ? &s->jmaps.sig[s->sig_cur] : nullptr, s->stream);
+                                  tma ? &s->jmaps.sig[s->sig_cur] : nullptr, &quad, s->stream);
+            if (quad.nbx > 0)
+                launch_jacobi_quad(s->g, s->storage, ns, quad, s->sig[1 - s->sig_cur], k2, &s->jmaps.rho[s->cur],
+                                   &s->jmaps.b, &s->jmaps.sig[s->sig_cur], s->stream);
             s->sig_cur = 1 - s->sig_cur;
         }
         launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);

@@ -52,8 +52,13 @@ template <typename T, int NS, int CPT>
 __global__ void __launch_bounds__(R * R / CPT, 1)
 k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ CUtensorMap bmap,
                  const __grid_constant__ CUtensorMap smap, int use_tma, Grid g, const T *__restrict__ rho,
-                 const float *__restrict__ bsrc, const T *__restrict__ sin, T *__restrict__ sout, float k2, int zc)
+                 const float *__restrict__ bsrc, const T *__restrict__ sin, T *__restrict__ sout, float k2, int zc,
+                 JacobiQuadPlan skip)
 {
+    // regions taken by k_jacobi_quad (CTA-uniform)
+    if ((int)blockIdx.x >= skip.bx0 && (int)blockIdx.x < skip.bx0 + skip.nbx && (int)blockIdx.y >= skip.by0 &&
+        (int)blockIdx.y < skip.by0 + skip.nby)
+        return;
     constexpr int OT = R - 2 * NS;
     constexpr int NTHREADS = R * R / CPT;
     constexpr int P = R + 2;                 // padded plane pitch: a border of one cell, so that the
@@ -390,7 +395,7 @@ int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_st
 template <typename T>
 static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, const void *sin, void *sout,
                       float k2, const CUtensorMap *rmap, const CUtensorMap *bmap, const CUtensorMap *smap,
-                      cudaStream_t st)
+                      const JacobiQuadPlan &skip, cudaStream_t st)
 {
     const int ot = R - 2 * ns, zc = jacobi_blocked_zc(g, ns);
     dim3 grid((g.nx + ot - 1) / ot, (g.ny + ot - 1) / ot, (g.nz + zc - 1) / zc);
@@ -409,7 +414,7 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
             configured = true;                                                                           \
         }                                                                                                \
         k_jacobi_blocked<T, NSV, CPTV><<<grid, R * R / CPTV, smem, st>>>(rm, bm, sm, use_tma, g, (const T *)rho, b, \
-                                                                    (const T *)sin, (T *)sout, k2, zc);  \
+                                                                    (const T *)sin, (T *)sout, k2, zc, skip);  \
     } while (0)
     switch (ns) {
     case 1: IGR_JB(1); break;
@@ -426,9 +431,17 @@ static void launch_ns(const Grid &g, int ns, const void *rho, const float *b, co
 // sig_in) regions inside the domain stage their planes by TMA; NULL maps: cp.async everywhere.
 void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, const float *b,
                            const void *sig_in, void *sig_out, float k2, const CUtensorMap *rmap,
-                           const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st)
+                           const CUtensorMap *bmap, const CUtensorMap *smap, const JacobiQuadPlan *skip,
+                           cudaStream_t st)
 {
-    if (storage == 0) launch_ns<float>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
-    else if (storage == 1) launch_ns<__half>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
-    else launch_ns<__nv_bfloat16>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, st);
+    JacobiQuadPlan none = {};
+    const JacobiQuadPlan &sk = skip ? *skip : none;
+    if (sk.nbx > 0 && sk.nby > 0) {
+        // every region is taken by the quad kernel: nothing to launch
+        const int ot = R - 2 * ns;
+        if (sk.bx0 == 0 && sk.by0 == 0 && sk.nbx >= (g.nx + ot - 1) / ot && sk.nby >= (g.ny + ot - 1) / ot) return;
+    }
+    if (storage == 0) launch_ns<float>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, sk, st);
+    else if (storage == 1) launch_ns<__half>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, sk, st);
+    else launch_ns<__nv_bfloat16>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, sk, st);
 }

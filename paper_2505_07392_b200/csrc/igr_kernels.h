@@ -63,6 +63,16 @@ struct JacobiMaps {
 };
 int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
                      const float *b, JacobiMaps *out);
+// a3 (quad form, igr_jacobi_quad.cu): the same blocked pass for the regions (bx, by), bx0 <= bx < bx0 + nbx,
+// by0 <= by < by0 + nby, that need no periodic wrap in x / y; four y-adjacent columns per thread.  nbx = 0: none.
+struct JacobiQuadPlan {
+    int bx0, by0, nbx, nby, zc;
+};
+JacobiQuadPlan jacobi_quad_plan(const Grid &g, int ns, float k2);
+void launch_jacobi_quad(const Grid &g, int storage, int ns, const JacobiQuadPlan &pl, void *sig_out, float k2,
+                        const CUtensorMap *rmap, const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st);
+// `skip` (may be NULL): regions of that plan are left to launch_jacobi_quad
 void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, const float *b,
                            const void *sig_in, void *sig_out, float k2, const CUtensorMap *rmap,
-                           const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st);
+                           const CUtensorMap *bmap, const CUtensorMap *smap, const JacobiQuadPlan *skip,
+                           cudaStream_t st);
