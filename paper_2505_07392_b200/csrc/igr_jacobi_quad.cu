@@ -22,13 +22,12 @@
 #include "igr_tma.cuh"
 
 #include <cuda.h>
+#include <cstdlib>
 #include <type_traits>
 
 namespace {
 
 constexpr int R = 32;                       // region edge = warp width
-constexpr int QR = 4;                       // rows per thread
-constexpr int NW = R / QR;                  // warps per CTA
 constexpr int PF = 3;                       // planes in flight (TMA)
 constexpr int NSLOT = PF + 2;               // + the plane that enters and the one before (its halo rows are still read)
 constexpr int SUB = (R + 4) * R;            // floats of one staged field: a box of (R + 16 bytes) x R
@@ -41,13 +40,15 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
-template <typename T, int NS>
-__global__ void __launch_bounds__(R * NW, 1)
+// QR = rows per thread (4: 8 warps x 255 registers; 2: 16 warps x 128 registers)
+template <typename T, int NS, int QR>
+__global__ void __launch_bounds__(R * (R / QR), 1)
 k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ CUtensorMap bmap,
               const __grid_constant__ CUtensorMap smap, Grid g, T *__restrict__ sout, float k2, int zc,
               int bx0, int by0, int nbx, int nby)
 {
     constexpr int OT = R - 2 * NS;
+    constexpr int NW = R / QR;                             // warps per CTA
     constexpr int NL = NS > 1 ? NS - 1 : 1;                // levels whose edge rows are exchanged
     extern __shared__ __align__(128) float jq_smem[];
     float *STG = jq_smem;                                                       // [NSLOT][3][SUB]
@@ -83,20 +84,24 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
     const int own_t = row0 * BWT + shT + lane, own_b = row0 * BWB + shB + lane;
     const int up_t = max(row0 - 1, 0) * BWT + shT + lane;          // row above / below the quad (own row at the
     const int dn_t = min(row0 + QR, R - 1) * BWT + shT + lane;     // region edge: outside the dependency cone)
-    // one thread: the next plane of the three fields -> a staging slot.  The z indices of that plane (rho keeps
-    // the first ghost layer: its density enters the face weights; b and Sigma follow the index map) are
-    // running counters: no division in the march.
-    int pn = 0, zwrap = 0;                       // next plane to issue; its wrapped index (periodic z)
-    auto tma_issue = [&](int stage) {
+    // one elected lane of warp 0: plane p of the three fields -> a staging slot.  Everything it needs is
+    // warp-uniform (uniform registers, no broadcast loops): the z index of the plane is a running counter kept
+    // by all threads (periodic z: wrapped; otherwise rho keeps the first ghost layer, whose density enters the
+    // face weights, and b, Sigma follow the index map).
+    const int wu = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    auto elect_one = []() {
+        uint32_t pred;
+        asm volatile("{\n .reg .pred P;\n elect.sync _|P, 0xffffffff;\n selp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+        return pred != 0;
+    };
+    auto tma_issue = [&](int p, int pwrap, int stage) {
         float *st = STG + stage * 3 * SUB;
-        const int zr = (per_z ? zwrap : min(max(pn, -1), g.nz)) + IGR_NG;
-        const int zm = (per_z ? zwrap : min(max(pn, 0), g.nz - 1)) + IGR_NG;
+        const int zr = (per_z ? pwrap : min(max(p, -1), g.nz)) + IGR_NG;
+        const int zm = (per_z ? pwrap : min(max(p, 0), g.nz - 1)) + IGR_NG;
         igr_tma::mbar_expect_tx(&full[stage], R * (2 * BWT * (int)sizeof(T) + BWB * 4));
         igr_tma::tma_load_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo, zr, &full[stage]);
         igr_tma::tma_load_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo, zm, &full[stage]);
         igr_tma::tma_load_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
-        ++pn;
-        if (++zwrap == g.nz) zwrap = 0;
     };
 
     // edge rows of the quads, levels 1 .. NS-1, double-buffered by plane parity: [par][l - 1][warp][top | bottom][32].
@@ -160,14 +165,17 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
     // range): Sigma_i = (b_i/K + sum_n W_in Sigma_n) / (1/(K rho_i) + sum_n W_in), W_in = 1/(rho_i + rho_n).
     const float k22 = 2.0f * k2, ik22 = 1.0f / k22;
     const int nsteps_r = (nsteps + NS - 1) / NS * NS;       // whole groups: the surplus steps load valid planes
+    int zwrap = kfirst % g.nz;               // wrapped index of the next plane to issue (periodic z)
+    if (zwrap < 0) zwrap += g.nz;
     if (threadIdx.x == 0) {
         for (int d = 0; d < NSLOT; ++d) igr_tma::mbar_init(&full[d], 1);
         igr_tma::fence_init();
-        pn = kfirst;
-        zwrap = kfirst % g.nz; if (zwrap < 0) zwrap += g.nz;
-        for (int d = 0; d < PF; ++d) tma_issue(d);                     // nsteps > PF always
     }
     __syncthreads();
+    for (int d = 0; d < PF; ++d) {                                     // nsteps > PF always
+        if (wu == 0 && elect_one()) tma_issue(kfirst + d, zwrap, d);
+        if (++zwrap == g.nz) zwrap = 0;
+    }
 
     const uint32_t full_s = igr_tma::smem_u32(full);
     unsigned slot = 0, phase = 0;            // staging slot of plane p0
@@ -185,11 +193,14 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
             const int tau = base + u;
             const int p0 = kfirst + tau, p1 = p0 - 1;
             // the slot of plane p0 + PF held plane p0 - 2, last read in the previous step (barrier since)
-            if (threadIdx.x == 0 && tau + PF < nsteps_r) {
-                igr_tma::fence_async();
+            if (wu == 0 && tau + PF < nsteps_r) {
                 unsigned fs = slot + PF; if (fs >= NSLOT) fs -= NSLOT;
-                tma_issue(fs);
+                if (elect_one()) {
+                    igr_tma::fence_async();
+                    tma_issue(p0 + PF, zwrap, fs);
+                }
             }
+            if (++zwrap == g.nz) zwrap = 0;
             igr_tma::mbar_wait_s32(full_s + 8u * slot, phase);
             const float *st0 = STG + slot * (3 * SUB);
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
@@ -314,19 +325,19 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
     }
 }
 
-template <typename T, int NS>
+template <typename T, int NS, int QR>
 void launch_quad(const Grid &g, const JacobiQuadPlan &pl, void *sout, float k2, const CUtensorMap &rm,
                  const CUtensorMap &bm, const CUtensorMap &sm, cudaStream_t st)
 {
-    constexpr int NL = NS > 1 ? NS - 1 : 1;
+    constexpr int NL = NS > 1 ? NS - 1 : 1, NW = R / QR;
     constexpr int smem = (NSLOT * 3 * SUB + NL * 2 * NW * 2 * 32) * 4 + NSLOT * 8 + 8;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_jacobi_quad<T, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaFuncSetAttribute(k_jacobi_quad<T, NS, QR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         configured = true;
     }
     const int nch = (g.nz + pl.zc - 1) / pl.zc;
-    k_jacobi_quad<T, NS><<<pl.nbx * pl.nby * nch, R * NW, smem, st>>>(rm, bm, sm, g, (T *)sout, k2, pl.zc, pl.bx0,
+    k_jacobi_quad<T, NS, QR><<<pl.nbx * pl.nby * nch, R * NW, smem, st>>>(rm, bm, sm, g, (T *)sout, k2, pl.zc, pl.bx0,
                                                                       pl.by0, pl.nbx, pl.nby);
 }
 
@@ -371,7 +382,15 @@ void launch_jacobi_quad(const Grid &g, int storage, int ns, const JacobiQuadPlan
                         const CUtensorMap *rmap, const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st)
 {
     if (pl.nbx <= 0 || ns != 5) return;
-    if (storage == 0) launch_quad<float, 5>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);
-    else if (storage == 1) launch_quad<__half, 5>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);
-    else launch_quad<__nv_bfloat16, 5>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);
+    static int qr = -1;                          // IGR_JACOBI_QR=2|4: rows per thread (tuning)
+    if (qr < 0) { const char *e = getenv("IGR_JACOBI_QR"); qr = (e && atoi(e) == 2) ? 2 : 4; }
+#define IGR_JQ(TT)                                                                         \
+    do {                                                                                   \
+        if (qr == 2) launch_quad<TT, 5, 2>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);   \
+        else launch_quad<TT, 5, 4>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);           \
+    } while (0)
+    if (storage == 0) IGR_JQ(float);
+    else if (storage == 1) IGR_JQ(__half);
+    else IGR_JQ(__nv_bfloat16);
+#undef IGR_JQ
 }
