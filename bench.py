@@ -8,7 +8,7 @@ A "step" is one pass of the whole hot path (halo/BC, source, Jacobi, RHS, RK upd
 the synthetic many-jet workload (config 5 of BASELINE.json at N=1).  Prints ONE JSON line.
 metric = grind time ns/(cell*eqn*RHS) = t_step / (cells * 5 * 3); lower is better.
 Multi-GPU (--gpus N under torchrun, one rank per GPU): weak scaling by z slabs: the
-job is the workload stacked N times along z, every rank owns one copy's planes plus 8 overlap planes per
+job is the workload stacked N times along z, every rank owns one copy's planes plus n_jacobi + 3 overlap planes per
 neighbour and pulls its halo planes from the neighbours after every RK stage (CUDA IPC peer copies, or
 torch.distributed send/recv); value = time / (total OWNED cells * 15), time = max over ranks.
 """
@@ -156,9 +156,25 @@ def alg_bytes(row, storage, fused=1):
 # + cell wave speeds 15 + divergence 30 + RK stage 20; jacobi = 5 sweeps x 14 + coefficients 20;
 # source = 9 differences + velocities + traces.
 ALG_FLOP = {"sigma_source": 45.0, "jacobi": 90.0, "rhs": 614.0, "rk_update": 20.0}
-# DRAM bytes per cell per launch measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum,
-# profiles/r01_ncu_full_*): fp32 storage, stage-1 launch of the fused RHS kernel
-NCU_DRAM_BYTES_PER_CELL = {"f32": {"sigma_source": 21.2, "jacobi": 21.4, "rhs": 47.6}}
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+
+
+def ncu_traffic(workload, storage, row):
+    """DRAM bytes per launch of `row` (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+    capture, profiles/dram_traffic.md), averaged over the launches of one step that were captured -- or None
+    if profiles/dram_traffic.csv holds no capture of exactly this workload and storage type.  Nothing is
+    scaled from another size."""
+    import csv
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, None
+    vals = []
+    with open(TRAFFIC_CSV) as f:
+        for r in csv.DictReader(line for line in f if not line.startswith("#")):
+            if r["workload"] == workload and r["storage"] == storage and r["row"] == row:
+                vals.append((float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]), r["stage"]))
+    if not vals:
+        return None, None
+    return sum(v for v, _ in vals) / len(vals), "+".join(st for _, st in vals)
 
 
 def alu_peak_tflops():
@@ -209,7 +225,7 @@ def run_ours(args):
     ss = None
     if world > 1:
         # z-slab decomposition: the job is the workload stacked `world` times along z,
-        # every rank owns w.nz planes and computes 8 overlap planes per neighbour on top of them
+        # every rank owns w.nz planes and computes n_jacobi + 3 overlap planes per neighbour on top of them
         import dataclasses
         from paper_2505_07392_b200 import dist as D, slab as S
         wg = dataclasses.replace(w, name="%s_x%dz" % (w.name, world), nz=w.nz * world)
@@ -247,6 +263,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     resets = [0]
+    resets_timed = [0]                    # restarts that fell between the two timing events
     solver = ss if ss else g              # max_wavespeed (max over ranks) and step (+ exchange per stage)
 
     dt_cache = [None, 0]                  # dt in use, steps since it was computed
@@ -279,9 +296,11 @@ def run_ours(args):
     l0 = g.kernel_launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(g.stream)
+    r_before = resets[0]
     for _ in range(args.steps):
         one_step()
     e1.record(g.stream)
+    resets_timed[0] = resets[0] - r_before
     barrier()
     ms = e0.elapsed_time(e1)
     launches = g.kernel_launches() - l0
@@ -327,9 +346,11 @@ def run_ours(args):
     else:
         roofline = {"bound": "hbm", "kernel": dom, "achieved": hbm_gbs[dom], "peak": peak, "unit": "GB/s",
                     "frac": hbm_gbs[dom] / peak, "peak_source": peak_src}
-    t_cell = NCU_DRAM_BYTES_PER_CELL.get(args.storage, {}).get(dom)
+    traffic, traffic_stages = (None, None) if ss else ncu_traffic(w.name, args.storage, dom)
     roofline.update({
-        "traffic": t_cell * cells if t_cell else None, "traffic_unit": "bytes per launch (ncu, see profiles/)",
+        "traffic": traffic,
+        "traffic_unit": ("bytes per launch, mean of the captured stages %s (ncu --set full, profiles/dram_traffic.csv)"
+                         % traffic_stages) if traffic else "no ncu capture of this workload / storage in profiles/",
         "alg_bytes_per_cell": alg_bytes(dom, args.storage, args.fused),
         "hbm": {"achieved_gbs": hbm_gbs[dom], "peak_gbs": peak, "frac": hbm_gbs[dom] / peak, "peak_source": peak_src,
                 "frac_of_nominal_8tbs": hbm_gbs[dom] / 8000.0},
@@ -369,18 +390,23 @@ def run_ours(args):
 
     out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "storage_dtype": args.storage, "data": "synthetic",
            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
                       "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
                       "cfl": w.cfl,
-                      "parallelism": ("z slabs: %d ranks x %d owned planes + 8 overlap planes per neighbour, one halo "
-                                      "exchange per RK stage (%s)" % (world, w.nz, ss.exchange_kind)) if ss else "single GPU",
+                      "parallelism": ("z slabs: %d ranks x %d owned planes + %d overlap planes per neighbour, one halo "
+                                      "exchange per RK stage (%s)" % (world, w.nz, ss.slab.overlap, ss.exchange_kind))
+                      if ss else "single GPU",
                       "exchange_ms_per_step": (t_ex[0] * 1e3 / nprof) if ss else 0.0,
                       "l2": "inputs larger than L2 (no flush needed)" if cells * 4 > (126 << 20) else "inputs fit L2",
                       "wavespeed_query_every_step": args.wavespeed_every == 1, "wavespeed_every": args.wavespeed_every,
                       "resets": resets[0]},
            "cell_updates_per_s": job["cell_updates_per_s"],
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+    if resets_timed[0]:
+        # the state was reloaded inside the timed region (positivity lost, F1): the line is flagged
+        out["invalid"] = "%d restart(s) from the initial state inside the timed region" % resets_timed[0]
+        print("bench.py: WARNING: " + out["invalid"], file=sys.stderr)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w)
     if rank == 0:

@@ -81,10 +81,13 @@ typedef struct {
 
 typedef struct {
     int32_t storage;       /* IGR_STORE_*                                                         */
-    int32_t fused;         /* 0: one kernel per row of the hot path (source, Jacobi, RHS, update)  */
-                           /* 1: RK update fused into the RHS kernel (one more state buffer)       */
-    int32_t variant;       /* IGR_VARIANT_TILED (default): TMA-staged tiled kernels;               */
-                           /* IGR_VARIANT_SIMPLE: one-thread-per-cell reference kernels (debugging) */
+    int32_t fused;         /* 1 (what igr_create uses): RK update and stage-3 wave speed fused into */
+                           /*    the RHS kernel (one more state buffer, no r array at rest)        */
+                           /* 0: one kernel per row of the hot path (source, Jacobi, RHS, update)  */
+    int32_t variant;       /* IGR_VARIANT_TILED (default): TMA-staged tiled kernels: the product;  */
+                           /* IGR_VARIANT_SIMPLE: TEST-ONLY one-thread-per-cell kernels, one launch */
+                           /*    per Jacobi sweep -- the first correct path, kept as a cross-check  */
+                           /*    of the tiled kernels against the oracle; never timed, not tuned    */
     int32_t reserved;
     void   *stream;        /* cudaStream_t to run on (NULL: the legacy default stream)             */
     void   *workspace;     /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-B     */
@@ -98,17 +101,22 @@ typedef struct igr_solver igr_solver;
  * igr_get_rhs or a viscous step needs it (IGR_ERR_ALLOC if that fails). */
 size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt);
 
-/* Create a solver.  dx: uniform spacing in all directions; gamma > 1: ideal-gas exponent (eq. 4);
+/* Create a solver (igr_create: fp32 storage, fused = 1, tiled kernels, default stream, library-owned memory).
+ * dx: uniform spacing in all directions; gamma > 1: ideal-gas exponent (eq. 4);
  * alpha >= 0: IGR strength, shock width ~ sqrt(alpha) (L130; the configs use 10 dx^2);
  * order: 5 (L132) or 3; n_jacobi >= 0 sweeps per RHS evaluation (L130 "<~ 10"; configs: 5).
- * Errors: IGR_ERR_ARG, IGR_ERR_BC, IGR_ERR_ALLOC, IGR_ERR_CUDA.  *out is NULL on failure. */
+ * Errors: IGR_ERR_ARG (also: a padded field of more than 2^32 - 1 elements, the kernels index cells with
+ * 32-bit offsets), IGR_ERR_BC, IGR_ERR_ALLOC, IGR_ERR_CUDA.  *out is NULL on failure. */
 int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
                int n_jacobi, const igr_bc *bc, igr_solver **out);
 int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
                   int n_jacobi, const igr_bc *bc, const igr_options *opt, igr_solver **out);
 void igr_destroy(igr_solver *s);
 
-/* Copy a state in (rounding to the storage format) and reset Sigma = 0 ("Sigma = 0 at t = 0"). */
+/* Copy a state in (rounding to the storage format) and reset Sigma = 0 ("Sigma = 0 at t = 0").
+ * q (here and in every other call that takes a field): host or device pointer, BORROWED FOR THE DURATION OF
+ * THE CALL ONLY: when the call returns a host buffer has been read completely (the library waits for its last
+ * host-to-device copy) and may be reused or freed; device buffers are read in stream order. */
 int igr_set_state(igr_solver *s, const float *q);
 /* Copy the current state out; synchronises.  IGR_ERR_NONFINITE is NOT raised here. */
 int igr_get_state(igr_solver *s, float *q);

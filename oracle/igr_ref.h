@@ -14,10 +14,14 @@
  * 60/61 (P6), uniform state bitwise (P7), conservation (P8), scale covariance (P9),
  * entropy-wave convergence order (P10), Sod vs exact Riemann solution (P11), axis
  * permutation symmetry (P12), periodic-doubling and inflow mask (P13); viscous fluxes
- * (NEXT-1): textbook stress cases, tau:grad u heating, discrete shear-wave decay (P14).
+ * (NEXT-1): textbook stress cases, tau:grad u heating, discrete shear-wave decay (P14);
+ * the CFL wave speed against its closed form (P15); the cell-centred sound speed and the
+ * local LF speed inside igr_ref_rhs against the textbook Rusanov flux worked out by hand
+ * beside a density jump (P16).  tests/test_oracle_f1.py records what the scheme as read
+ * does on the inputs as BASELINE.json states them (finding F1).
  * Parity unpinned by any external value (fixed by DESIGN.md readings A2-A5 only):
- * the 5-sweep truncation, the warm-start order, the choice of the LF wave speed and
- * the arithmetic-mean face density.
+ * the 5-sweep truncation, the warm-start order, the CHOICE of the local cell-centred LF
+ * speed (its formula is pinned by P16) and the arithmetic-mean face density.
  *
  * Layout: every field is a padded array [nz+2*NG][ny+2*NG][nx+2*NG], x fastest,
  * NG = 3 ghost layers on every side.  State q = (rho, m_x, m_y, m_z, E).

@@ -188,6 +188,9 @@ int field_in(igr_solver *s, const float *user, void *field, int storage, int kfi
         IGR_CUDA_OK(cudaMemcpyAsync(s->stage, user + (size_t)k0 * g.nx * g.ny, nk * plane,
                                     cudaMemcpyHostToDevice, s->stream));
         launch_unpack_field(g, storage, s->stage, field, kfirst + k0, nk, s->stream);
+        // the staging buffer is reused by the next chunk and `user` is borrowed for the duration of the call
+        // only (igr.h): the copy must have left the host buffer before this returns
+        IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
     }
     return IGR_OK;
 }
@@ -259,7 +262,7 @@ size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt)
 {
     if (nx < 1 || ny < 1 || nz < 1) return 0;
     const int storage = opt ? opt->storage : IGR_STORE_F32;
-    const int fused = opt ? opt->fused : 0;
+    const int fused = opt ? opt->fused : 1;
     if (storage < 0 || storage > 2) return 0;
     Grid g = make_grid(nx, ny, nz, storage, nullptr);
     return make_layout(g, storage, fused, opt ? opt->variant : 0).total;
@@ -292,7 +295,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
 
     igr_solver *s = new igr_solver();
     s->storage = storage;
-    s->fused = opt ? (opt->fused != 0) : 0;
+    s->fused = opt ? (opt->fused != 0) : 1;                 // igr_create: the fused (headline) path
     s->variant = opt ? opt->variant : 0;
     s->maps.valid = false;
     s->jmaps.valid = false;
@@ -300,6 +303,10 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
     s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
     s->g = make_grid(nx, ny, nz, storage, bc->face);
+    if (s->g.np > (long long)UINT32_MAX) {       // the kernels address cells with 32-bit unsigned element offsets
+        delete s;
+        return IGR_ERR_ARG;
+    }
     const Layout L = make_layout(s->g, storage, s->fused, s->variant);
     if (opt && opt->workspace) {
         if (opt->workspace_bytes < L.total || ((uintptr_t)opt->workspace % kAlign) != 0) {
@@ -591,9 +598,11 @@ int igr_rk_update(igr_solver *s, int stage, double dt)
     if (stage == 1) {
         launch_rk_update(s->g, s->storage, A, A, B, s->r, beta, (float)dt, (float)s->gamma, nullptr, s->stream);
         s->cur = 1;
+        s->wave_valid = false;                   // the cached speed is the one of q^n, not of this sub-step
     } else if (stage == 2) {
         launch_rk_update(s->g, s->storage, A, B, B, s->r, beta, (float)dt, (float)s->gamma, nullptr, s->stream);
         s->cur = 1;
+        s->wave_valid = false;
     } else {
         IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
         launch_rk_update(s->g, s->storage, A, B, A, s->r, beta, (float)dt, (float)s->gamma, s->wave, s->stream);
@@ -647,7 +656,7 @@ int igr_stage(igr_solver *s, int stage, double dt)
                 launch_viscous_tile(s->g, s->storage, s->order, true, s->vmaps.q[src], s->vmaps.tau, v, s->stream);
             }
             s->cur = dst;
-            if (stage == 3) s->wave_valid = true;
+            s->wave_valid = stage == 3;          // the cached speed belongs to q^n / q^{n+1} only
             if ((rc = finish(s, "igr_step (fused rhs)")) != IGR_OK) return rc;
         } else {
             if ((rc = igr_rhs(s)) != IGR_OK) return rc;
@@ -794,8 +803,11 @@ int igr_set_viscosity(igr_solver *s, double mu, double zeta)
         IGR_CUDA_OK(cudaMemsetAsync(s->tau, 0, (size_t)s->g.np * 6 * 4, s->stream));
         if (s->variant == IGR_VARIANT_TILED) {
             const char *msg = "";
-            if (visc_tile_make_maps(s->g, s->storage, s->st, 3, s->tau, &s->vmaps, &msg) != 0)
+            if (visc_tile_make_maps(s->g, s->storage, s->st, 3, s->tau, &s->vmaps, &msg) != 0) {
+                cudaFree(s->tau);                // a later call must not find stress fields without maps
+                s->tau = nullptr;
                 return s->fail(IGR_ERR_CUDA, msg);
+            }
         }
     }
     s->mu = mu; s->zeta = zeta;

@@ -152,7 +152,7 @@ class Solver:
     """igr_create_ex / igr_destroy and the calls of include/igr.h on one solver object."""
 
     def __init__(self, nx, ny, nz, dx, gamma, alpha, order=5, n_jacobi=5, faces=(0,) * 6, patches=None,
-                 storage=STORE_F32, fused=0, variant=VARIANT_TILED, device="cuda:0", own_workspace=True):
+                 storage=STORE_F32, fused=1, variant=VARIANT_TILED, device="cuda:0", own_workspace=True):
         L = lib()
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)

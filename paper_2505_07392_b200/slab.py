@@ -5,20 +5,19 @@ Host logic only: index arithmetic, no arithmetic of the method.  Used by the mul
 
 Scheme (reading A20).  The global grid is cut into N slabs of whole z-planes (z is the
 slowest axis of the padded layout: a range of planes is ONE contiguous chunk per field, so the exchange
-needs no pack kernels).  A rank's local solver works on its owned planes EXTENDED by `OVERLAP` = 8 planes
+needs no pack kernels).  A rank's local solver works on its owned planes EXTENDED by `overlap` planes
 on every side that has a neighbour; those faces carry the BC code EXTERNAL (ghosts are not filled by
 the solver).  One RK stage computed on the extended slab is exact on the owned planes: the only wrong
 inputs are the Sigma neighbours beyond the extended boundary, they contaminate one more plane per
-Jacobi sweep (5), and the flux stencil reaches 3 planes: 5 + 3 = 8.  After every stage each rank
-overwrites its overlap and ghost planes (8 + 3 = 11 per side, q and Sigma) with the neighbour's owned
-planes.  Redundant work: 16 planes per rank (1.6 % at 1024 planes).  The result on the owned planes is
-bitwise the single-domain result."""
+Jacobi sweep, and the flux stencil reaches 3 planes: overlap = n_jacobi + 3 (8 with the 5 sweeps of every
+configuration; `overlap_for`).  After every stage each rank overwrites its overlap and ghost planes
+(overlap + 3 per side, q and Sigma) with the neighbour's owned planes.  Redundant work: 2 x overlap planes
+per rank (1.6 % at 1024 planes).  The result on the owned planes is bitwise the single-domain result."""
 from dataclasses import dataclass, replace
 
 from .workloads import Workload, _state_slab
 
-OVERLAP = 8          # planes of redundant computation per side with a neighbour
-NG = 3               # ghost layers
+NG = 3               # ghost layers = planes the flux stencil reaches
 EXTERNAL = 3         # BC code of a face shared with a neighbour (include/igr.h IGR_BC_EXTERNAL)
 PERIODIC = 0
 
@@ -35,6 +34,7 @@ class Slab:
     hi: int
     local: Workload      # the workload the local solver is created for (nz = e1 - e0)
     nz_global: int
+    overlap: int = 0     # planes of redundant computation per side with a neighbour
 
     @property
     def own_lo(self):    # local index of the first owned plane
@@ -46,7 +46,13 @@ class Slab:
 
     @property
     def halo(self):      # planes received per side
-        return OVERLAP + NG
+        return self.overlap + NG
+
+
+def overlap_for(w):
+    """Planes of redundant computation per side with a neighbour: one per Jacobi sweep (the sweeps clamp at the
+    extended boundary, the error moves one plane per sweep) plus the reach of the flux stencil."""
+    return w.n_jacobi + NG
 
 
 def split(nz, nranks):
@@ -60,12 +66,15 @@ def split(nz, nranks):
     return out
 
 
-def make_slab(w, rank, nranks, overlap=OVERLAP):
-    """The slab of global workload `w` owned by `rank` of `nranks`."""
+def make_slab(w, rank, nranks, overlap=None):
+    """The slab of global workload `w` owned by `rank` of `nranks`.  `overlap` defaults to `overlap_for(w)`;
+    a smaller value is accepted only so that the tests can show that the bound is sharp."""
     assert 0 <= rank < nranks
+    if overlap is None:
+        overlap = overlap_for(w)
     periodic = w.faces[4] == PERIODIC
     if nranks == 1:
-        return Slab(0, 1, 0, w.nz, 0, w.nz, -1, -1, w, w.nz)
+        return Slab(0, 1, 0, w.nz, 0, w.nz, -1, -1, w, w.nz, overlap)
     z0, z1 = split(w.nz, nranks)[rank]
     sizes = [b - a for a, b in split(w.nz, nranks)]
     assert min(sizes) >= overlap + NG, "slabs thinner than %d planes cannot feed their neighbours" % (overlap + NG)
@@ -87,7 +96,7 @@ def make_slab(w, rank, nranks, overlap=OVERLAP):
     gshape = w.global_shape or (w.nx, w.ny, w.nz)
     local = replace(w, name="%s_slab%dof%d" % (w.name, rank, nranks), nz=e1 - e0, faces=tuple(faces),
                     patches=patches, origin=(w.origin[0], w.origin[1], w.origin[2] + e0), global_shape=gshape)
-    return Slab(rank, nranks, z0, z1, e0, e1, lo, hi, local, w.nz)
+    return Slab(rank, nranks, z0, z1, e0, e1, lo, hi, local, w.nz, overlap)
 
 
 def local_state(w, slab, device="cpu", dtype=None):

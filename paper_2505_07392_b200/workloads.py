@@ -144,15 +144,18 @@ def _state_slab(w, device, dtype, kz0, nk):
         # primitive state blends from the patch state to the ambient with a tanh profile of
         # half-width `delta` cells about the patch edge; by default the columns run through the
         # whole domain height (no impulsive-start vortex ring), else up to z = stub_height.
+        # stub_delta = 0 is the configuration AS BASELINE.json STATES IT: grid-sharp patches (edge 0) into gas
+        # at rest, no columns -- kept so that the tests can show where the scheme loses positivity on it.
         delta = P["stub_delta"]
         gx, gy, gz = gi.to(f64) + 0.5, gj.to(f64) + 0.5, gk.to(f64) + 0.5
         h = P.get("stub_height")               # None: columns through the whole domain
-        sz = 1.0 if h is None else 0.5 * (1.0 - torch.tanh((gz - h) / delta))
         s = torch.zeros((1, w.ny, w.nx), dtype=f64, device=dev)
-        for cx, cy, rad in P["jet_centers"]:          # GLOBAL cell units (sub-box independent)
-            rr = torch.sqrt((gx - cx) ** 2 + (gy - cy) ** 2)
-            s = torch.maximum(s, 0.5 * (1.0 - torch.tanh((rr - rad) / delta)))
-        s = s * sz
+        if delta > 0:
+            sz = 1.0 if h is None else 0.5 * (1.0 - torch.tanh((gz - h) / delta))
+            for cx, cy, rad in P["jet_centers"]:          # GLOBAL cell units (sub-box independent)
+                rr = torch.sqrt((gx - cx) ** 2 + (gy - cy) ** 2)
+                s = torch.maximum(s, 0.5 * (1.0 - torch.tanh((rr - rad) / delta)))
+            s = s * sz
         rho_j, w_j, p_j = P["jet_state"]
         rho = 1.0 + (rho_j - 1.0) * s
         p = 1.0 + (p_j - 1.0) * s

@@ -51,6 +51,39 @@ def test_config2_sod_l1_vs_oracle_and_exact(shape, mode):
     assert l1_exact <= (1e-2 if nx >= 512 else 2.5e-2), l1_exact
 
 
+def test_config2_as_stated_gpu_follows_the_oracle_until_both_lose_positivity():
+    """Finding F1 on the GPU (tests/test_oracle_f1.py holds the oracle side): config 2 with the grid-sharp
+    interface of BASELINE.json.  The GPU must follow the oracle on harsh data too: element-wise parity at the
+    shocked-case tolerance (L1-rel <= 1e-3) after every step while the state is still positive, and
+    IGR_ERR_NONFINITE reported at the step at which the oracle's pressure goes negative."""
+    w = W.sod(256, 8, 8, smooth=0.0)
+    q0 = W.state(w).numpy()
+    p0 = np.round(q0[4, 0, 0].astype(np.float64) * 0.4, 5)
+    assert sorted(set(p0.tolist())) == [0.1, 1.0] and p0[127] == 1.0 and p0[128] == 0.1   # one-cell interface
+    g = igr.Solver.for_workload(w, **BENCH_MODE)
+    ref = parity.oracle_for(w)
+    g.set_state(q0); ref.set_state(q0.astype(np.float64))
+    gpu_fail = ref_fail = None
+    for n in range(30):
+        qr = ref.get_state()
+        pr = 0.4 * (qr[4] - 0.5 * (qr[1] ** 2 + qr[2] ** 2 + qr[3] ** 2) / qr[0])
+        if not (np.isfinite(qr).all() and qr[0].min() > 0 and pr.min() > 0):
+            ref_fail = n
+        try:
+            lam = g.max_wavespeed()
+        except igr.IgrError as e:
+            assert e.code == igr.ERR_NONFINITE
+            gpu_fail = n
+        if gpu_fail is not None or ref_fail is not None:
+            break
+        mx, l1 = parity.worst(g.get_state(), qr)
+        assert l1 <= 1e-3, (n, mx, l1)
+        dt = w.cfl * w.dx / lam
+        g.step(dt); ref.step(dt)
+    assert ref_fail is not None and 8 <= ref_fail <= 12, ref_fail
+    assert gpu_fail == ref_fail, (gpu_fail, ref_fail)
+
+
 @pytest.mark.parametrize("n,mode", [(64, m) for m in MODES] + ([(256, "tiled_fused")] if FULL else []))
 def test_config3_taylor_green_first_5_steps(n, mode):
     w = W.taylor_green(n)

@@ -55,10 +55,15 @@ def exchange_in_process(slabs, refs):
             r.set_padded(c, p[c])
 
 
-@pytest.mark.parametrize("case,nranks", [("jets", 2), ("jets", 3), ("tg_periodic", 2), ("tg_periodic", 3)])
-def test_slabs_with_stage_exchange_equal_the_global_run_bitwise(case, nranks):
+@pytest.mark.parametrize("case,nranks,n_jacobi", [("jets", 2, 5), ("jets", 3, 5), ("tg_periodic", 2, 5),
+                                                   ("tg_periodic", 3, 5), ("jets", 2, 7), ("tg_periodic", 2, 3)])
+def test_slabs_with_stage_exchange_equal_the_global_run_bitwise(case, nranks, n_jacobi):
+    """The overlap follows the sweep count (slab.overlap_for: n_jacobi + 3): 7 sweeps need 10 planes, 3 need 6."""
+    import dataclasses
     w = small_jets() if case == "jets" else periodic_tg()
+    w = dataclasses.replace(w, n_jacobi=n_jacobi)
     slabs = [S.make_slab(w, r, nranks) for r in range(nranks)]
+    assert all(sl.overlap == n_jacobi + 3 and sl.halo == n_jacobi + 6 for sl in slabs)
     refs = []
     for sl in slabs:
         r = parity.oracle_for(sl.local)
