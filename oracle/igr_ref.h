@@ -112,6 +112,43 @@ void igr_ref_viscous_flux(int d, double mu, double zeta, const double *G9, const
 /* round x to the storage format (round to nearest even)                               */
 double igr_ref_round_storage(double x, int mode);
 
+/* ---------------------------------------------------------------- two-fluid variant (NEXT-3)
+ * igr_ref2.c: five-equation (volume-fraction) model of two ideal gases, reading A21; see the header of that
+ * file for the passages of the paper it follows and for its pins.  State layout [7][nz][ny][nx]:
+ * (a1 rho1, a2 rho2, rho u, rho v, rho w, E, a1). */
+typedef struct {
+    double c0, c1, radius, edge;          /* as igr_ref_patch                                  */
+    double a1rho1, a2rho2, a1;            /* partial densities and volume fraction of fluid 1  */
+    double u, v, w, p;
+} igr_ref2_patch;
+
+typedef struct {
+    int face[6];                          /* periodic / extrapolation / inflow                 */
+    int n_patches[6];
+    const igr_ref2_patch *patches[6];
+} igr_ref2_bc;
+
+typedef struct igr_ref2_solver igr_ref2_solver;
+
+int  igr_ref2_create(int nx, int ny, int nz, double dx, double gamma1, double gamma2, double alpha, int order,
+                     int n_jacobi, const igr_ref2_bc *bc, igr_ref2_solver **out);
+void igr_ref2_destroy(igr_ref2_solver *s);
+int  igr_ref2_set_state(igr_ref2_solver *s, const double *q);     /* also resets Sigma = 0 */
+int  igr_ref2_get_state(const igr_ref2_solver *s, double *q);
+int  igr_ref2_get_rhs(const igr_ref2_solver *s, double *r);       /* last computed r [7]... */
+int  igr_ref2_get_sigma(const igr_ref2_solver *s, double *sig);
+int  igr_ref2_set_sigma(igr_ref2_solver *s, const double *sig);
+int  igr_ref2_get_source(const igr_ref2_solver *s, double *b);
+int  igr_ref2_get_padded(const igr_ref2_solver *s, int c, double *out);   /* c = 0..6, 7 = Sigma */
+int  igr_ref2_max_wavespeed(const igr_ref2_solver *s, double *out);
+int  igr_ref2_step(igr_ref2_solver *s, double dt);
+int  igr_ref2_stage(igr_ref2_solver *s, int stage, double dt);
+int  igr_ref2_fill_ghosts(igr_ref2_solver *s);
+int  igr_ref2_source(igr_ref2_solver *s);
+int  igr_ref2_solve_sigma(igr_ref2_solver *s);
+int  igr_ref2_rhs(igr_ref2_solver *s);
+int  igr_ref2_eval_rhs(igr_ref2_solver *s);
+
 #ifdef __cplusplus
 }
 #endif
