@@ -71,6 +71,9 @@ typedef enum {
 typedef struct {
     double c0, c1, radius, edge;
     double rho, u, v, w, p;
+    double a1, rho2;              /* two fluids only (igr_options.n_fluids = 2): volume fraction of fluid 1 and   */
+                                  /* density of fluid 2 in the patch; `rho` is then the density of fluid 1:      */
+                                  /* q_fixed = (a1 rho, (1 - a1) rho2, rho_m u, rho_m v, rho_m w, E, a1)         */
 } igr_patch;
 
 typedef struct {
@@ -88,10 +91,18 @@ typedef struct {
                            /* IGR_VARIANT_SIMPLE: TEST-ONLY one-thread-per-cell kernels, one launch */
                            /*    per Jacobi sweep -- the first correct path, kept as a cross-check  */
                            /*    of the tiled kernels against the oracle; never timed, not tuned    */
-    int32_t reserved;
+    int32_t n_fluids;      /* 0 or 1: one ideal gas (the hot path).  2: the TWO-FLUID variant (SURVEY 8(f)  */
+                           /*    NEXT-3; Alg. 1; reading A21): the      */
+                           /*    five-equation model of two ideal gases (gamma of igr_create_ex and gamma2), */
+                           /*    state [7][nz][ny][nx] = (a1 rho1, a2 rho2, rho u, rho v, rho w, E, a1),     */
+                           /*    p = (E - rho |u|^2/2)/Gamma, Gamma = a1/(gamma-1) + (1-a1)/(gamma2-1);     */
+                           /*    fp32 storage, order 5, fused tiled kernels only (else IGR_ERR_ARG); no      */
+                           /*    viscosity, no slabs.  Every call that takes or returns "the state" then     */
+                           /*    moves 7 fields, igr_get_padded takes c = 0..7 (7 = Sigma)                   */
     void   *stream;        /* cudaStream_t to run on (NULL: the legacy default stream)             */
     void   *workspace;     /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-B     */
     size_t  workspace_bytes; /* aligned, at least igr_workspace_bytes(); NULL: library allocates  */
+    double  gamma2;        /* n_fluids = 2: ideal-gas exponent of fluid 2 (> 1)                    */
 } igr_options;
 
 typedef struct igr_solver igr_solver;

@@ -45,7 +45,7 @@ struct Layout {
     size_t total;
 };
 
-Layout make_layout(const Grid &g, int storage, int fused, int variant)
+Layout make_layout(const Grid &g, int storage, int fused, int variant, int nf = 5)
 {
     Layout L;
     L.q_bytes = align_up((size_t)g.np * elem_size(storage), kAlign);
@@ -54,8 +54,10 @@ Layout make_layout(const Grid &g, int storage, int fused, int variant)
     // the fused tiled step never materialises r: it is allocated only if an unfused row, igr_get_rhs or
     // the viscous path asks for it (5 fp32 fields less: 18 instead of 23 fields at rest)
     L.n_r = (fused && variant == IGR_VARIANT_TILED) ? 0 : 5;
-    // states + Sigma x2 (storage type) + b + r[n_r] (fp32) + staging + wave result
-    L.total = (size_t)L.n_state * 5 * L.q_bytes + 2 * L.q_bytes + (1 + L.n_r) * L.f_bytes + kStageBytes + kAlign;
+    // states + Sigma x2 (storage type) + b + r[n_r] (fp32) + staging + wave result (+ the mixture density with
+    // two fluids)
+    L.total = (size_t)L.n_state * nf * L.q_bytes + 2 * L.q_bytes + (1 + L.n_r + (nf == 7 ? 1 : 0)) * L.f_bytes +
+              kStageBytes + kAlign;
     return L;
 }
 
@@ -67,6 +69,9 @@ struct igr_solver {
     RhsTileMaps maps;
     JacobiMaps jmaps;                // TMA maps of the blocked Jacobi kernel
     double dx = 0, gamma = 0, alpha = 0;
+    int nf = 5;                      // conserved fields: 5, or 7 with two fluids (NEXT-3, reading A21)
+    double gamma2 = 0;               // two fluids: exponent of fluid 2
+    float *rhot = nullptr;           // two fluids: mixture density of every padded cell (fp32)
     cudaStream_t stream = nullptr;
     char *base = nullptr;            // device memory (owned or caller's workspace)
     bool owns_base = false;
@@ -133,7 +138,8 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
         const int a = f / 2;
         F.n0 = (a == 0) ? n[1] : n[0];
         F.n1 = (a == 2) ? n[1] : n[2];
-        std::vector<float> w((size_t)F.n0 * F.n1), fx((size_t)F.n0 * F.n1 * 5, 0.f);
+        const int nf = s->nf;
+        std::vector<float> w((size_t)F.n0 * F.n1), fx((size_t)F.n0 * F.n1 * nf, 0.f);
         for (int t1 = 0; t1 < F.n1; ++t1)
             for (int t0 = 0; t0 < F.n0; ++t0) {
                 double best = 0.0; const igr_patch *bp = nullptr;
@@ -145,11 +151,17 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
                 w[id] = (float)best;
                 if (best >= 1.0) w[id] = 1.0f;
                 else if (best > 0.0 && w[id] >= 1.0f) w[id] = 0.99999994f;   // keep "w < 1" in fp32
-                if (bp) {
+                if (bp && nf == 5) {
                     const double ke = 0.5 * bp->rho * (bp->u * bp->u + bp->v * bp->v + bp->w * bp->w);
                     const double v[5] = { bp->rho, bp->rho * bp->u, bp->rho * bp->v, bp->rho * bp->w,
                                           bp->p / (s->gamma - 1.0) + ke };
                     for (int c = 0; c < 5; ++c) fx[id * 5 + c] = (float)v[c];
+                } else if (bp) {             // two fluids (igr.h, igr_patch): rho = fluid 1, rho2 = fluid 2
+                    const double m1 = bp->a1 * bp->rho, m2 = (1.0 - bp->a1) * bp->rho2, rm = m1 + m2;
+                    const double ke = 0.5 * rm * (bp->u * bp->u + bp->v * bp->v + bp->w * bp->w);
+                    const double G = bp->a1 / (s->gamma - 1.0) + (1.0 - bp->a1) / (s->gamma2 - 1.0);
+                    const double v[7] = { m1, m2, rm * bp->u, rm * bp->v, rm * bp->w, bp->p * G + ke, bp->a1 };
+                    for (int c = 0; c < 7; ++c) fx[id * 7 + c] = (float)v[c];
                 }
             }
         float *dw = nullptr, *dfx = nullptr;
@@ -265,7 +277,7 @@ size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt)
     const int fused = opt ? opt->fused : 1;
     if (storage < 0 || storage > 2) return 0;
     Grid g = make_grid(nx, ny, nz, storage, nullptr);
-    return make_layout(g, storage, fused, opt ? opt->variant : 0).total;
+    return make_layout(g, storage, fused, opt ? opt->variant : 0, (opt && opt->n_fluids == 2) ? 7 : 5).total;
 }
 
 int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
@@ -293,7 +305,16 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return IGR_ERR_CUDA; }
 
+    const bool two = opt && opt->n_fluids == 2;
+    if (opt && (opt->n_fluids < 0 || opt->n_fluids > 2)) return IGR_ERR_ARG;
+    // two fluids (NEXT-3): fp32 storage, order 5, fused tiled kernels only
+    if (two && (storage != IGR_STORE_F32 || order != 5 || !opt->fused || opt->variant != IGR_VARIANT_TILED ||
+                !(opt->gamma2 > 1)))
+        return IGR_ERR_ARG;
+
     igr_solver *s = new igr_solver();
+    s->nf = two ? 7 : 5;
+    s->gamma2 = two ? opt->gamma2 : 0.0;
     s->storage = storage;
     s->fused = opt ? (opt->fused != 0) : 1;                 // igr_create: the fused (headline) path
     s->variant = opt ? opt->variant : 0;
@@ -307,7 +328,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
         delete s;
         return IGR_ERR_ARG;
     }
-    const Layout L = make_layout(s->g, storage, s->fused, s->variant);
+    const Layout L = make_layout(s->g, storage, s->fused, s->variant, s->nf);
     if (opt && opt->workspace) {
         if (opt->workspace_bytes < L.total || ((uintptr_t)opt->workspace % kAlign) != 0) {
             delete s;
@@ -326,11 +347,12 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     if (cudaMemsetAsync(s->base, 0, L.total, s->stream) != cudaSuccess) { igr_destroy(s); return IGR_ERR_CUDA; }
     char *p = s->base;
     for (int b = 0; b < L.n_state; ++b)
-        for (int c = 0; c < 5; ++c) { s->st[b].f[c] = p; p += L.q_bytes; }
+        for (int c = 0; c < s->nf; ++c) { s->st[b].f[c] = p; p += L.q_bytes; }
     if (L.n_state < 3) s->st[2] = s->st[1];
     s->sig[0] = p; p += L.q_bytes;
     s->sig[1] = p; p += L.q_bytes;
     s->b = (float *)p; p += L.f_bytes;
+    if (two) { s->rhot = (float *)p; p += L.f_bytes; }
     for (int c = 0; c < L.n_r; ++c) { s->r[c] = (float *)p; p += L.f_bytes; }
     s->stage = (float *)p; p += kStageBytes;
     s->wave = (WaveResult *)p;
@@ -338,11 +360,14 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     if (rc != IGR_OK) { igr_destroy(s); return rc; }
     if (s->variant == IGR_VARIANT_TILED) {
         const char *msg = "";
-        if (rhs_tile_make_maps(s->g, storage, s->st, L.n_state, s->sig, &s->maps, &msg) != 0) {
+        if (rhs_tile_make_maps(s->g, storage, s->st, L.n_state, s->sig, s->nf, &s->maps, &msg) != 0) {
             igr_destroy(s);
             return IGR_ERR_CUDA;
         }
-        if (jacobi_make_maps(s->g, storage, s->st, L.n_state, s->sig, s->b, &s->jmaps) != 0) {
+        // the density the Sigma equation reads: field 0 of the state, or the mixture density (two fluids)
+        StagePtrs rho_of[3];
+        for (int b = 0; b < 3; ++b) { rho_of[b] = s->st[b]; if (two) rho_of[b].f[0] = s->rhot; }
+        if (jacobi_make_maps(s->g, storage, rho_of, L.n_state, s->sig, s->b, &s->jmaps) != 0) {
             igr_destroy(s);
             return IGR_ERR_CUDA;
         }
@@ -377,7 +402,7 @@ int igr_set_state(igr_solver *s, const float *q)
     if (!s || !q) return IGR_ERR_ARG;
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
     s->cur = 0;
-    for (int c = 0; c < 5; ++c) {
+    for (int c = 0; c < s->nf; ++c) {
         int rc = field_in(s, q + c * n, s->st[0].f[c], s->storage);
         if (rc != IGR_OK) return rc;
     }
@@ -394,7 +419,7 @@ int igr_set_state_planes(igr_solver *s, int k0, int nk, const float *q)
     if (!s || !q || k0 < 0 || nk < 1 || k0 + nk > s->g.nz) return IGR_ERR_ARG;
     if (s->cur != 0) return s->fail(IGR_ERR_ARG, "igr_set_state_planes: called in the middle of a step");
     const size_t n = (size_t)s->g.nx * s->g.ny * nk;
-    for (int c = 0; c < 5; ++c) {
+    for (int c = 0; c < s->nf; ++c) {
         int rc = field_in(s, q + c * n, s->st[0].f[c], s->storage, k0, nk);
         if (rc != IGR_OK) return rc;
     }
@@ -406,7 +431,7 @@ int igr_get_state_planes(igr_solver *s, int k0, int nk, float *q)
 {
     if (!s || !q || k0 < 0 || nk < 1 || k0 + nk > s->g.nz) return IGR_ERR_ARG;
     const size_t n = (size_t)s->g.nx * s->g.ny * nk;
-    for (int c = 0; c < 5; ++c) {
+    for (int c = 0; c < s->nf; ++c) {
         int rc = field_out(s, s->st[s->cur].f[c], q + c * n, s->storage, k0, nk);
         if (rc != IGR_OK) return rc;
     }
@@ -417,7 +442,7 @@ int igr_get_state(igr_solver *s, float *q)
 {
     if (!s || !q) return IGR_ERR_ARG;
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
-    for (int c = 0; c < 5; ++c) {
+    for (int c = 0; c < s->nf; ++c) {
         int rc = field_out(s, s->st[s->cur].f[c], q + c * n, s->storage);
         if (rc != IGR_OK) return rc;
     }
@@ -460,6 +485,7 @@ int igr_set_source(igr_solver *s, const float *f)
 int igr_get_rhs(igr_solver *s, float *r)
 {
     if (!s || !r) return IGR_ERR_ARG;
+    if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: r is never materialised (fused step only)");
     { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
     for (int c = 0; c < 5; ++c) {
@@ -471,9 +497,9 @@ int igr_get_rhs(igr_solver *s, float *r)
 
 int igr_get_padded(igr_solver *s, int c, float *f)
 {
-    if (!s || !f || c < 0 || c > 5) return IGR_ERR_ARG;
+    if (!s || !f || c < 0 || c > s->nf) return IGR_ERR_ARG;
     const Grid &g = s->g;
-    const void *field = c < 5 ? s->st[s->cur].f[c] : s->sig[s->sig_cur];
+    const void *field = c < s->nf ? s->st[s->cur].f[c] : s->sig[s->sig_cur];
     const size_t wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG, wz = g.nz + 2 * IGR_NG;
     if (is_device_pointer(f)) {
         launch_pack_padded(g, s->storage, field, f, 0, (int)wz, s->stream);
@@ -497,16 +523,23 @@ int igr_halo_bc(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     RowTimer t(s, 0, 1);
-    launch_halo_q(s->g, s->storage, s->st[s->cur], s->bc, s->stream);
+    launch_halo_q(s->g, s->storage, s->st[s->cur], s->bc, s->nf, s->stream);
     return finish(s, "igr_halo_bc");
 }
 
 int igr_sigma_source(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
-    RowTimer t(s, 1, 1);
+    RowTimer t(s, 1, s->nf == 7 ? 2 : 1);
     const bool viscous = s->mu > 0 || s->zeta > 0;
-    launch_source(s->g, s->storage, s->st[s->cur], s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
+    StagePtrs q = s->st[s->cur];
+    if (s->nf == 7) {
+        // two fluids: the mixture density of every padded cell first; the source kernel then sees
+        // (rho, m_x, m_y, m_z) as with one fluid
+        launch_rho_total(s->g, (const float *)q.f[0], (const float *)q.f[1], s->rhot, s->stream);
+        q.f[0] = s->rhot; q.f[1] = s->st[s->cur].f[2]; q.f[2] = s->st[s->cur].f[3]; q.f[3] = s->st[s->cur].f[4];
+    }
+    launch_source(s->g, s->storage, q, s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
                   viscous ? s->tau : nullptr, (float)s->mu, (float)s->zeta, s->stream);
     return finish(s, "igr_sigma_source");
 }
@@ -532,7 +565,7 @@ int igr_jacobi(igr_solver *s)
             // the blocked kernel keeps the others
             JacobiQuadPlan quad = {};
             if (tma && !no_quad) quad = jacobi_quad_plan(s->g, ns, k2);
-            launch_jacobi_blocked(s->g, s->storage, ns, s->st[s->cur].f[0], s->b,
+            launch_jacobi_blocked(s->g, s->storage, ns, s->nf == 7 ? (void *)s->rhot : s->st[s->cur].f[0], s->b,
                                   s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2,
                                   tma ? &s->jmaps.rho[s->cur] : nullptr, tma ? &s->jmaps.b : nullptr,
                                   tma ? &s->jmaps.sig[s->sig_cur] : nullptr, &quad, s->stream);
@@ -546,7 +579,7 @@ int igr_jacobi(igr_solver *s)
     }
     RowTimer t(s, 2, s->n_jacobi + 1);
     for (int it = 0; it < s->n_jacobi; ++it) {
-        launch_jacobi_sweep(s->g, s->storage, s->st[s->cur].f[0], s->b, s->sig[s->sig_cur],
+        launch_jacobi_sweep(s->g, s->storage, s->nf == 7 ? (void *)s->rhot : s->st[s->cur].f[0], s->b, s->sig[s->sig_cur],
                             s->sig[1 - s->sig_cur], k2, s->stream);
         s->sig_cur = 1 - s->sig_cur;
     }
@@ -557,6 +590,7 @@ int igr_jacobi(igr_solver *s)
 int igr_rhs(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
+    if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: only the fused step (igr_step / igr_stage) is built");
     { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     RowTimer t(s, 3, 1);
     RhsParams p;
@@ -591,6 +625,7 @@ int igr_rhs(igr_solver *s)
 int igr_rk_update(igr_solver *s, int stage, double dt)
 {
     if (!s || stage < 1 || stage > 3) return IGR_ERR_ARG;
+    if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: only the fused step (igr_step / igr_stage) is built");
     { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     const float beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
     StagePtrs &A = s->st[0], &B = s->st[1];
@@ -636,8 +671,10 @@ int igr_stage(igr_solver *s, int stage, double dt)
             if (stage == 3) IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
             RhsTileArgs a = {};
             a.gamma = (float)s->gamma; a.inv_dx = (float)(1.0 / s->dx); a.zc = 0;
+            a.nf = s->nf;
+            if (s->nf == 7) { a.k1 = (float)(1.0 / (s->gamma - 1.0)); a.k2 = (float)(1.0 / (s->gamma2 - 1.0)); }
             if (!viscous) {
-                for (int c = 0; c < 5; ++c) { a.qn[c] = s->st[0].f[c]; a.qout[c] = s->st[dst].f[c]; }
+                for (int c = 0; c < s->nf; ++c) { a.qn[c] = s->st[0].f[c]; a.qout[c] = s->st[dst].f[c]; }
                 a.beta = beta; a.dt = (float)dt; a.read_qn = stage != 1;
                 if (stage == 3) a.wave = s->wave;
                 launch_rhs_tile(s->g, s->storage, s->order, true, s->maps.q[src], s->maps.sig[s->sig_cur], a, s->stream);
@@ -682,6 +719,7 @@ int igr_step(igr_solver *s, double dt)
 int igr_export_fields(igr_solver *s, igr_export *out)
 {
     if (!s || !out) return IGR_ERR_ARG;
+    if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: the slab exchange is not built");
     memset(out, 0, sizeof *out);
     out->base = (uint64_t)(uintptr_t)s->base;
     for (int b = 0; b < 3; ++b)
@@ -775,7 +813,11 @@ int igr_max_wavespeed(igr_solver *s, double *out)
     if (!s->wave_valid) {
         RowTimer t(s, 5, 1);
         IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
-        launch_wavespeed(s->g, s->storage, s->st[s->cur], (float)s->gamma, s->wave, s->stream);
+        if (s->nf == 7)
+            launch_wavespeed2(s->g, s->st[s->cur], (float)(1.0 / (s->gamma - 1.0)), (float)(1.0 / (s->gamma2 - 1.0)),
+                              s->wave, s->stream);
+        else
+            launch_wavespeed(s->g, s->storage, s->st[s->cur], (float)s->gamma, s->wave, s->stream);
         s->wave_valid = (s->cur == 0);
     }
     WaveResult h;
@@ -794,6 +836,7 @@ int igr_max_wavespeed(igr_solver *s, double *out)
 int igr_set_viscosity(igr_solver *s, double mu, double zeta)
 {
     if (!s || !(mu >= 0) || !(zeta >= 0)) return IGR_ERR_ARG;
+    if (s->nf != 5 && (mu > 0 || zeta > 0)) return s->fail(IGR_ERR_ARG, "two fluids: viscous fluxes are not built");
     if ((mu > 0 || zeta > 0) && !s->tau) {
         if (cudaMalloc((void **)&s->tau, (size_t)s->g.np * 6 * 4) != cudaSuccess) {
             cudaGetLastError();

@@ -54,8 +54,8 @@ __device__ __forceinline__ void stf(float *p, float v) { *p = v; }
 __device__ __forceinline__ void stf(__half *p, float v) { *p = __float2half_rn(v); }
 __device__ __forceinline__ void stf(__nv_bfloat16 *p, float v) { *p = __float2bfloat16_rn(v); }
 
-struct StagePtrs {            // device pointers of one state buffer (5 padded fields)
-    void *f[5];
+struct StagePtrs {            // device pointers of one state buffer (5 padded fields; 7 with two fluids)
+    void *f[7];
 };
 
 // inflow description of one face, device resident (weights precomputed on the host in fp64)
@@ -89,6 +89,23 @@ __device__ __forceinline__ float wavespeed_of(float rho, float mx, float my, flo
     const float c = __fsqrt_rn(__fmul_rn(__fmul_rn(gamma, p), ir));
     const float v = __fmaf_rn(fmaxf(fabsf(mx), fmaxf(fabsf(my), fabsf(mz))), fabsf(ir), c);
     // non-finite (NaN/Inf, or sqrt of a negative) is reported, never repaired (reading A10)
+    if (!(v <= 3.0e38f)) { bad = true; return 0.f; }
+    return v;
+}
+
+// the same for two fluids (reading A21): q = (a1 rho1, a2 rho2, m, E, a1), c^2 = (1 + 1/Gamma) p / rho,
+// Gamma = a1 k1 + (1 - a1) k2, k_i = 1/(gamma_i - 1)
+__device__ __forceinline__ float wavespeed_of2(const float *q, float k1, float k2, bool &bad)
+{
+    const float rho = __fadd_rn(q[0], q[1]);
+    const float ir = __fdiv_rn(1.0f, rho);
+    float m2 = __fmul_rn(q[2], q[2]);
+    m2 = __fmaf_rn(q[3], q[3], m2);
+    m2 = __fmaf_rn(q[4], q[4], m2);
+    const float g1 = __fdiv_rn(1.0f, __fmaf_rn(q[6], k1 - k2, k2));
+    const float p = __fmul_rn(g1, __fmaf_rn(__fmul_rn(-0.5f, ir), m2, q[5]));
+    const float c = __fsqrt_rn(__fmul_rn(__fmul_rn(__fadd_rn(1.0f, g1), p), ir));
+    const float v = __fmaf_rn(fmaxf(fabsf(q[2]), fmaxf(fabsf(q[3]), fabsf(q[4]))), fabsf(ir), c);
     if (!(v <= 3.0e38f)) { bad = true; return 0.f; }
     return v;
 }

@@ -138,7 +138,7 @@ __host__ __device__ inline long long ghost_count(const Grid &g)
 }
 
 template <typename T>
-__global__ void k_halo_q(Grid g, StagePtrs q, BcDesc bc)
+__global__ void k_halo_q(Grid g, StagePtrs q, BcDesc bc, int nf)
 {
     const long long n = ghost_count(g);
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
@@ -162,10 +162,11 @@ __global__ void k_halo_q(Grid g, StagePtrs q, BcDesc bc)
             int t1 = (a == 2) ? idx[1] : idx[2];
             if (t0 < 0 || t0 >= f.n0 || t1 < 0 || t1 >= f.n1) continue;   // edge/corner ghosts: never read
             float ww = f.weight[(long long)t1 * f.n0 + t0];
-            if (ww > 0.f) { w = ww; fixed = f.fixed + ((long long)t1 * f.n0 + t0) * 5; }
+            if (ww > 0.f) { w = ww; fixed = f.fixed + ((long long)t1 * f.n0 + t0) * nf; }
         }
 #pragma unroll
-        for (int cmp = 0; cmp < 5; ++cmp) {
+        for (int cmp = 0; cmp < 7; ++cmp) {
+            if (cmp >= nf) break;
             T *fld = (T *)q.f[cmp];
             float v = ldf(fld + src);
             if (fixed != nullptr) v = (w >= 1.f) ? fixed[cmp] : v + w * (fixed[cmp] - v);
@@ -210,10 +211,24 @@ void launch_halo_fields(const Grid &g, float *base, int nf, cudaStream_t st)
     k_halo_fields<<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, base, nf);
 }
 
-void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cudaStream_t st)
+void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, int nf, cudaStream_t st)
 {
     long long n = ghost_count(g);
-    DISPATCH_STORAGE(storage, k_halo_q<T><<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, q, bc));
+    DISPATCH_STORAGE(storage, k_halo_q<T><<<blocks_for(n, 256, 148 * 16), 256, 0, st>>>(g, q, bc, nf));
+}
+
+// two fluids: mixture density rho = a1 rho1 + a2 rho2 of EVERY cell of the padded array (ghosts included: the
+// face weights of the Sigma equation read the first ghost layer), as one more fp32 field
+__global__ void k_rho_total(const float *__restrict__ r1, const float *__restrict__ r2, float *__restrict__ out,
+                            long long n)
+{
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x)
+        out[t] = __fadd_rn(r1[t], r2[t]);
+}
+
+void launch_rho_total(const Grid &g, const float *r1, const float *r2, float *out, cudaStream_t st)
+{
+    k_rho_total<<<blocks_for(g.np, 256, 148 * 16), 256, 0, st>>>(r1, r2, out, g.np);
 }
 
 void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st)
@@ -609,6 +624,32 @@ void launch_wavespeed(const Grid &g, int storage, StagePtrs q, float gamma, Wave
 {
     long long n = (long long)g.nx * g.ny * g.nz;
     DISPATCH_STORAGE(storage, k_wavespeed<T><<<blocks_for(n, 256, 148 * 8), 256, 0, st>>>(g, q, gamma, wave));
+}
+
+// two fluids (fp32 storage): mixture wave speed, reading A21
+__global__ void k_wavespeed2(Grid g, StagePtrs q, float k1, float k2, WaveResult *wave)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    float vmax = 0.f;
+    bool bad = false;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        if (k < g.wk0 || k >= g.wk1) continue;
+        const long long id = g.idx(i, j, k);
+        float v[7];
+#pragma unroll
+        for (int c = 0; c < 7; ++c) v[c] = ((const float *)q.f[c])[id];
+        vmax = fmaxf(vmax, wavespeed_of2(v, k1, k2, bad));
+    }
+    block_reduce_wave(vmax, bad, wave);
+}
+
+void launch_wavespeed2(const Grid &g, StagePtrs q, float k1, float k2, WaveResult *wave, cudaStream_t st)
+{
+    long long n = (long long)g.nx * g.ny * g.nz;
+    k_wavespeed2<<<blocks_for(n, 256, 148 * 8), 256, 0, st>>>(g, q, k1, k2, wave);
 }
 
 // ------------------------------------------------------------------------------ NEXT-1: viscous fluxes

@@ -23,7 +23,12 @@ void launch_pack_padded(const Grid &g, int storage, const void *field, float *us
                         cudaStream_t st);
 
 // a1: ghosts of q (5 fields) / of Sigma
-void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, cudaStream_t st);
+// (nf = 5 fields, or 7 with two fluids; the fixed inflow states hold nf values per transverse cell)
+void launch_halo_q(const Grid &g, int storage, StagePtrs q, const BcDesc &bc, int nf, cudaStream_t st);
+// two fluids (NEXT-3, reading A21; fp32 storage): mixture density of every cell of the padded array, and the
+// mixture wave speed
+void launch_rho_total(const Grid &g, const float *r1, const float *r2, float *out, cudaStream_t st);
+void launch_wavespeed2(const Grid &g, StagePtrs q, float k1, float k2, WaveResult *wave, cudaStream_t st);
 void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st);
 
 // a2: b = alpha (tr((grad u)^2) + (tr grad u)^2)

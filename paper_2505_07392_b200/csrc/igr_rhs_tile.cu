@@ -46,29 +46,31 @@ __device__ __forceinline__ float sqrt_fast(float x)
 }
 
 // ---- geometry of one ring slot for storage type T
-template <typename T, int TY, int NSLOT_OF_T = (sizeof(T) == 4 ? 7 : IGR_RHS_NSLOT_HALF)>
+// NF = conserved fields (5: single fluid; 7: two fluids, reading A21)
+template <typename T, int TY, int NF = 5, int NSLOT_OF_T = (sizeof(T) == 4 && NF == 5 ? 7 : IGR_RHS_NSLOT_HALF)>
 struct Tile {
+    static constexpr int NC = NF == 5 ? 5 : NF + 1;      // flux components exchanged per face (two fluids: + u^)
     static constexpr int NSLOT = NSLOT_OF_T;             // ring slots (planes): 4 live + 2 or 3 in flight
     static constexpr int HX = 16 / (int)sizeof(T);       // x halo of the box: 4 (fp32) / 8 (half) -> 16 B
     static constexpr int BX = TX + 2 * HX;               // box extents
     static constexpr int BY = TY + 6;
     static constexpr int PE = BX * BY;                   // elements of one field in a plane
-    static constexpr int QBYTES = (5 * PE * (int)sizeof(T) + 127) / 128 * 128;
+    static constexpr int QBYTES = (NF * PE * (int)sizeof(T) + 127) / 128 * 128;
     static constexpr int SBYTES = (PE * (int)sizeof(T) + 127) / 128 * 128;
     static constexpr int SLOT = QBYTES + SBYTES;          // bytes per slot
-    static constexpr int TXBYTES = 6 * PE * (int)sizeof(T); // bytes one plane's two TMA loads deliver
+    static constexpr int TXBYTES = (NF + 1) * PE * (int)sizeof(T); // bytes one plane's two TMA loads deliver
     static constexpr int AW = TX + 2;                     // width of the wave-speed arrays (halo 1)
     static constexpr int RING = NSLOT * SLOT;
     // everything below is double-buffered by plane / step parity: one __syncthreads per plane
     static constexpr int A_N = (TY + 2) * AW;                        // floats of one wave-speed array
     static constexpr int A_OFF = RING;                               // float [2][ax | ay][A_N]
-    static constexpr int FY_OFF = A_OFF + 2 * 2 * A_N * 4;           // float [2][5][TY][TX]
-    static constexpr int EX_OFF = FY_OFF + 2 * 5 * TY * TX * 4;      // float [2][5][TY]
-    static constexpr int EY_OFF = EX_OFF + 2 * 5 * TY * 4;           // float [2][5][TX]
+    static constexpr int FY_OFF = A_OFF + 2 * 2 * A_N * 4;           // float [2][NC][TY][TX]
+    static constexpr int EX_OFF = FY_OFF + 2 * NC * TY * TX * 4;     // float [2][NC][TY]
+    static constexpr int EY_OFF = EX_OFF + 2 * NC * TY * 4;          // float [2][NC][TX]
     // reduced-precision storage: the current plane is converted ONCE to fp32 (two buffers by plane
     // parity, same box layout, Sigma after the five q fields) so that the stencil taps need no cvt
-    static constexpr int CUR_N = (sizeof(T) == 2) ? 6 * PE : 0;      // floats per buffer
-    static constexpr int CUR_OFF = (EY_OFF + 2 * 5 * TX * 4 + 15) / 16 * 16;
+    static constexpr int CUR_N = (sizeof(T) == 2) ? (NF + 1) * PE : 0; // floats per buffer
+    static constexpr int CUR_OFF = (EY_OFF + 2 * NC * TX * 4 + 15) / 16 * 16;
     static constexpr int BAR_OFF = (CUR_OFF + 2 * CUR_N * 4 + 7) / 8 * 8;
     static constexpr int TOTAL = BAR_OFF + NSLOT * 8;
 };
@@ -108,68 +110,104 @@ __device__ __forceinline__ void recon(const float t[6], float &l, float &r)
     }
 }
 
-// physical flux of one side along D from reconstructed conservative values U[0..4] and Sigma U[5]
-template <int D>
-__device__ __forceinline__ void side_flux2(const float U[6], float gm1, float F[5])
-{
-    const float ir = rcp_fast(U[0]);
-    const float ud = __fmul_rn(U[1 + D], ir);
-    float m2 = __fmul_rn(U[1], U[1]);
-    m2 = __fmaf_rn(U[2], U[2], m2);
-    m2 = __fmaf_rn(U[3], U[3], m2);
-    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, U[4]);     // E - |m|^2/(2 rho)
-    const float pt = __fmaf_rn(gm1, e, U[5]);                      // p + Sigma
-    F[0] = U[1 + D];
-    F[1] = (D == 0) ? __fmaf_rn(U[1], ud, pt) : __fmul_rn(U[1], ud);
-    F[2] = (D == 1) ? __fmaf_rn(U[2], ud, pt) : __fmul_rn(U[2], ud);
-    F[3] = (D == 2) ? __fmaf_rn(U[3], ud, pt) : __fmul_rn(U[3], ud);
-    F[4] = __fmul_rn(__fadd_rn(U[4], pt), ud);
-}
+// Equation of state handed to the flux routines.  Single fluid: p = (gamma - 1) e.  Two fluids (reading A21): the
+// isobaric mixture rule p = e / Gamma, Gamma = a1/(gamma_1 - 1) + (1 - a1)/(gamma_2 - 1) = a1 (k1 - k2) + k2.
+struct Eos {
+    float gamma, gm1;      // single fluid
+    float k1, k2;          // two fluids: 1/(gamma_i - 1)
+};
 
-template <int ORDER, int D>
-__device__ __forceinline__ void face_flux2(const float t[6][6], float lam, float gm1, float G[5])
+// physical flux of one side along D from the reconstructed conservative values U[0..NF-1] and Sigma U[NF].
+// NF = 5: U = (rho, m, E), F = (m_d, m u_d + (p + Sigma) e_d, (E + p + Sigma) u_d)              (eqs. 6-8).
+// NF = 7: U = (a1 rho1, a2 rho2, m, E, a1), F = (a1 rho1 u_d, a2 rho2 u_d, ..., a1 u_d), and F[7] = u_d (for u^).
+template <int D, int NF>
+__device__ __forceinline__ void side_flux2(const float *U, const Eos &eos, float *F)
 {
-    float L[6], R[6];
-#pragma unroll
-    for (int f = 0; f < 6; ++f) recon<ORDER>(t[f], L[f], R[f]);
-    float FL[5], FR[5];
-    side_flux2<D>(L, gm1, FL);
-    side_flux2<D>(R, gm1, FR);
-#pragma unroll
-    for (int c = 0; c < 5; ++c)
-        G[c] = __fmaf_rn(-lam, __fsub_rn(R[c], L[c]), __fadd_rn(FL[c], FR[c]));
-}
-
-// cell-centred wave speeds |u_d| + c of one cell (reading A5); explicit intrinsics as above
-__device__ __forceinline__ void cell_speeds(float rho, float mx, float my, float mz, float E, float gamma,
-                                            float &ax, float &ay, float &az)
-{
+    constexpr int IM = NF == 5 ? 1 : 2, IE = IM + 3;
+    const float rho = NF == 5 ? U[0] : __fadd_rn(U[0], U[1]);
     const float ir = rcp_fast(rho);
-    float m2 = __fmul_rn(mx, mx);
-    m2 = __fmaf_rn(my, my, m2);
-    m2 = __fmaf_rn(mz, mz, m2);
-    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, E);
-    const float c = sqrt_fast(__fmul_rn(__fmul_rn(gamma, gamma - 1.0f), __fmul_rn(e, ir)));
-    ax = __fadd_rn(fabsf(__fmul_rn(mx, ir)), c);
-    ay = __fadd_rn(fabsf(__fmul_rn(my, ir)), c);
-    az = __fadd_rn(fabsf(__fmul_rn(mz, ir)), c);
+    const float ud = __fmul_rn(U[IM + D], ir);
+    float m2 = __fmul_rn(U[IM], U[IM]);
+    m2 = __fmaf_rn(U[IM + 1], U[IM + 1], m2);
+    m2 = __fmaf_rn(U[IM + 2], U[IM + 2], m2);
+    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, U[IE]);    // E - |m|^2/(2 rho)
+    float pt;                                                      // p + Sigma
+    if (NF == 5) {
+        pt = __fmaf_rn(eos.gm1, e, U[NF]);
+        F[0] = U[IM + D];
+    } else {
+        const float g1 = rcp_fast(__fmaf_rn(U[6], eos.k1 - eos.k2, eos.k2));   // 1 / Gamma(a1)
+        pt = __fmaf_rn(g1, e, U[NF]);
+        F[0] = __fmul_rn(U[0], ud);
+        F[1] = __fmul_rn(U[1], ud);
+        F[6] = __fmul_rn(U[6], ud);
+        F[7] = ud;
+    }
+    F[IM] = (D == 0) ? __fmaf_rn(U[IM], ud, pt) : __fmul_rn(U[IM], ud);
+    F[IM + 1] = (D == 1) ? __fmaf_rn(U[IM + 1], ud, pt) : __fmul_rn(U[IM + 1], ud);
+    F[IM + 2] = (D == 2) ? __fmaf_rn(U[IM + 2], ud, pt) : __fmul_rn(U[IM + 2], ud);
+    F[IE] = __fmul_rn(__fadd_rn(U[IE], pt), ud);
+}
+
+// G = 2 F^ for the NF conserved fields; two fluids: G[NF] = u_d,L + u_d,R = 2 u^ (the face velocity of a1 div u)
+template <int ORDER, int D, int NF>
+__device__ __forceinline__ void face_flux2(const float t[][6], float lam, const Eos &eos, float *G)
+{
+    constexpr int NC = NF == 5 ? 5 : NF + 1;
+    float L[NF + 1], R[NF + 1];
+#pragma unroll
+    for (int f = 0; f < NF + 1; ++f) recon<ORDER>(t[f], L[f], R[f]);
+    float FL[NC], FR[NC];
+    side_flux2<D, NF>(L, eos, FL);
+    side_flux2<D, NF>(R, eos, FR);
+#pragma unroll
+    for (int c = 0; c < NF; ++c)
+        G[c] = __fmaf_rn(-lam, __fsub_rn(R[c], L[c]), __fadd_rn(FL[c], FR[c]));
+    if (NF != 5) G[NF] = __fadd_rn(FL[NF], FR[NF]);
+}
+
+// cell-centred wave speeds |u_d| + c of one cell (reading A5); explicit intrinsics as above.
+// q[0..NF-1]: the conserved values of the cell.  c^2 = gamma p / rho, two fluids: (1 + 1/Gamma) p / rho.
+template <int NF>
+__device__ __forceinline__ void cell_speeds(const float *q, const Eos &eos, float &ax, float &ay, float &az)
+{
+    constexpr int IM = NF == 5 ? 1 : 2, IE = IM + 3;
+    const float rho = NF == 5 ? q[0] : __fadd_rn(q[0], q[1]);
+    const float ir = rcp_fast(rho);
+    float m2 = __fmul_rn(q[IM], q[IM]);
+    m2 = __fmaf_rn(q[IM + 1], q[IM + 1], m2);
+    m2 = __fmaf_rn(q[IM + 2], q[IM + 2], m2);
+    const float e = __fmaf_rn(__fmul_rn(-0.5f, ir), m2, q[IE]);
+    float gg;                                                      // gamma (gamma - 1), or (1 + 1/Gamma)/Gamma
+    if (NF == 5) gg = __fmul_rn(eos.gamma, eos.gm1);
+    else {
+        const float g1 = rcp_fast(__fmaf_rn(q[6], eos.k1 - eos.k2, eos.k2));
+        gg = __fmul_rn(__fadd_rn(1.0f, g1), g1);
+    }
+    const float c = sqrt_fast(__fmul_rn(gg, __fmul_rn(e, ir)));
+    ax = __fadd_rn(fabsf(__fmul_rn(q[IM], ir)), c);
+    ay = __fadd_rn(fabsf(__fmul_rn(q[IM + 1], ir)), c);
+    az = __fadd_rn(fabsf(__fmul_rn(q[IM + 2], ir)), c);
 }
 
 }  // namespace
 
 // ======================================================================================= kernel
-template <typename T, int TY, int ORDER, bool FUSE>
-__global__ void __launch_bounds__(TX * TY, (TY <= 8) ? 2 : 1)
+template <typename T, int TY, int ORDER, bool FUSE, int NF>
+__global__ void __launch_bounds__(TX * TY, (TY <= 8 && NF == 5) ? 2 : 1)
 k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap smap, Grid g,
            RhsTileArgs a)
 {
-    using TL = Tile<T, TY>;
+    using TL = Tile<T, TY, NF>;
+    constexpr int NC = TL::NC;                                          // flux components per face
+    constexpr int NW = NF + 1;                                          // fields in the window: q and Sigma
+    constexpr bool TWO = NF != 5;
     extern __shared__ __align__(1024) unsigned char smem[];
     float *Abase = reinterpret_cast<float *>(smem + TL::A_OFF);         // [2][ax | ay][(TY+2)][AW]
-    float *FYbase = reinterpret_cast<float *>(smem + TL::FY_OFF);       // [2][5][TY][TX]
-    float *EXbase = reinterpret_cast<float *>(smem + TL::EX_OFF);       // [2][5][TY]
-    float *EYbase = reinterpret_cast<float *>(smem + TL::EY_OFF);       // [2][5][TX]
-    float *CUR = reinterpret_cast<float *>(smem + TL::CUR_OFF);         // [2][6][PE] (half storage only)
+    float *FYbase = reinterpret_cast<float *>(smem + TL::FY_OFF);       // [2][NC][TY][TX]
+    float *EXbase = reinterpret_cast<float *>(smem + TL::EX_OFF);       // [2][NC][TY]
+    float *EYbase = reinterpret_cast<float *>(smem + TL::EY_OFF);       // [2][NC][TX]
+    float *CUR = reinterpret_cast<float *>(smem + TL::CUR_OFF);         // [2][NW][PE] (half storage only)
     constexpr bool HALF = sizeof(T) == 2;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + TL::BAR_OFF);
 
@@ -179,7 +217,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     const int nkz = min(a.zc, g.nz - kz0);
     const int i = x0 + tx, j = y0 + ty;
     const bool valid = (i < g.nx) && (j < g.ny);
-    const float gm1 = a.gamma - 1.0f;
+    Eos eos;
+    eos.gamma = a.gamma; eos.gm1 = a.gamma - 1.0f; eos.k1 = a.k1; eos.k2 = a.k2;
     const float hdx = 0.5f * a.inv_dx;                 // G = 2 F^
 
     // TMA coordinates of the box origin in the padded arrays (elements)
@@ -204,26 +243,32 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     auto sbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT + TL::QBYTES); };
 
     // ---- prologue: window of planes p = 0..5 (cells kz0-3 .. kz0+2), flux of the face kz0-1/2
-    float W[6][6];                                                 // W[f][s]
+    float W[NW][6];                                                // W[f][s]
 #pragma unroll
     for (int s = 0; s < 6; ++s) {
         mbar_wait(&full[s], 0);
         const T *qb = qbase(s) + own;
 #pragma unroll
-        for (int f = 0; f < 5; ++f) W[f][s] = lds<T>(qb + f * TL::PE);
-        W[5][s] = lds<T>(sbase(s) + own);
+        for (int f = 0; f < NF; ++f) W[f][s] = lds<T>(qb + f * TL::PE);
+        W[NF][s] = lds<T>(sbase(s) + own);
     }
-    float Gz_prev[5];
+    // the conserved values of the own column at window position s
+    auto column = [&](int s, float *q) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) q[f] = W[f][s];
+    };
+    float Gz_prev[NC];
     float ax_c, ay_c, az_c;
     {
-        float bx, by, bz, az_m;
-        cell_speeds(W[0][2], W[1][2], W[2][2], W[3][2], W[4][2], a.gamma, bx, by, az_m);   // cell kz0-1
-        cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_c, ay_c, az_c); // cell kz0
-        face_flux2<ORDER, 2>(W, fmaxf(az_m, az_c), gm1, Gz_prev);
-        (void)bx; (void)by; (void)bz;
+        float bx, by, az_m, q2[NF], q3[NF];
+        column(2, q2); column(3, q3);
+        cell_speeds<NF>(q2, eos, bx, by, az_m);                    // cell kz0-1
+        cell_speeds<NF>(q3, eos, ax_c, ay_c, az_c);                // cell kz0
+        face_flux2<ORDER, 2, NF>(W, fmaxf(az_m, az_c), eos, Gz_prev);
+        (void)bx; (void)by;
     }
 #pragma unroll
-    for (int f = 0; f < 6; ++f) {
+    for (int f = 0; f < NW; ++f) {
 #pragma unroll
         for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];          // now cells kz0-2 .. kz0+2 in W[.][0..4]
     }
@@ -241,9 +286,10 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
                 if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
                 else { const int hh = h - 2 * TY; hy = (hh >= TX) ? TY : -1; hx = hh & (TX - 1); }
                 const T *c0 = qp + (3 + hy) * TL::BX + TL::HX + hx;
-                float hax, hay, haz;
-                cell_speeds(lds<T>(c0), lds<T>(c0 + TL::PE), lds<T>(c0 + 2 * TL::PE), lds<T>(c0 + 3 * TL::PE),
-                            lds<T>(c0 + 4 * TL::PE), a.gamma, hax, hay, haz);
+                float hq[NF], hax, hay, haz;
+#pragma unroll
+                for (int f = 0; f < NF; ++f) hq[f] = lds<T>(c0 + f * TL::PE);
+                cell_speeds<NF>(hq, eos, hax, hay, haz);
                 A0[(hy + 1) * TL::AW + hx + 1] = hax;
                 A1[(hy + 1) * TL::AW + hx + 1] = hay;
             }
@@ -259,7 +305,7 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             if (std::is_same<T, __half>::value) return __half22float2(*reinterpret_cast<const __half2 *>(&v));
             return __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&v));
         };
-        constexpr int NT = TX * TY, NQ = 5 * TL::PE / 2, NSG = TL::PE / 2;       // pairs of q / of Sigma
+        constexpr int NT = TX * TY, NQ = NF * TL::PE / 2, NSG = TL::PE / 2;      // pairs of q / of Sigma
 #pragma unroll
         for (int it = 0; it < (NQ + NT - 1) / NT; ++it) {
             const int e = tid + it * NT;
@@ -297,21 +343,25 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         {
             const T *qb = qbase(slot_n) + own;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) W[f][5] = lds<T>(qb + f * TL::PE);
-            W[5][5] = lds<T>(sbase(slot_n) + own);
+            for (int f = 0; f < NF; ++f) W[f][5] = lds<T>(qb + f * TL::PE);
+            W[NF][5] = lds<T>(sbase(slot_n) + own);
         }
         // fused update: q^n of this cell is fetched now and consumed at the end of the step, so that
         // the global-load latency hides behind the flux computation
-        float qn_pre[5];
+        float qn_pre[NF];
         const unsigned id = uid;                                    // element offset of cell (i, j, kz0 + t)
         uid += (unsigned)g.sz;
         if (FUSE && a.read_qn) {                                   // (columns beyond the domain read a valid
 #pragma unroll                                                      //  cell: the offset is clamped, nothing is stored)
-            for (int c = 0; c < 5; ++c) qn_pre[c] = ldf(reinterpret_cast<const T *>(a.qn[c]) + id);
+            for (int c = 0; c < NF; ++c) qn_pre[c] = ldf(reinterpret_cast<const T *>(a.qn[c]) + id);
         }
         // wave speeds of the next cell (k+1) of this column, published for the next step
         float ax_n, ay_n, az_n;
-        cell_speeds(W[0][3], W[1][3], W[2][3], W[3][3], W[4][3], a.gamma, ax_n, ay_n, az_n);
+        {
+            float q3[NF];
+            column(3, q3);
+            cell_speeds<NF>(q3, eos, ax_n, ay_n, az_n);
+        }
         put_speeds(pc + 1, slot_c1, ax_n, ay_n);                  // read in the next step (after the barrier)
         convert_plane(pc + 1, slot_c1);
         // the current plane as seen by the stencil taps: the ring slot itself (fp32) or its fp32 copy
@@ -319,65 +369,65 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         const TC *qc = HALF ? reinterpret_cast<const TC *>(CUR + (pc & 1) * TL::CUR_N)
                             : reinterpret_cast<const TC *>(qbase(slot_c));
         const float *A0 = Abase + (pc & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
-        float *FY = FYbase + (t & 1) * 5 * TY * TX, *EX = EXbase + (t & 1) * 5 * TY, *EY = EYbase + (t & 1) * 5 * TX;
+        float *FY = FYbase + (t & 1) * NC * TY * TX, *EX = EXbase + (t & 1) * NC * TY, *EY = EYbase + (t & 1) * NC * TX;
 
-        const TC *sc = HALF ? qc + 5 * TL::PE : reinterpret_cast<const TC *>(sbase(slot_c));
-        float Gx[5], Gy[5];
+        const TC *sc = HALF ? qc + NF * TL::PE : reinterpret_cast<const TC *>(sbase(slot_c));
+        float Gx[NC], Gy[NC];
         {   // x+ face of the own cell: cells i-2 .. i+3
-            float tp[6][6];
+            float tp[NW][6];
             const TC *qb = qc + own;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) {
+            for (int f = 0; f < NF; ++f) {
 #pragma unroll
                 for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2));
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<TC>(sc + own + (s - 2));
-            face_flux2<ORDER, 0>(tp, fmaxf(ax_c, A0[(ty + 1) * TL::AW + tx + 2]), gm1, Gx);
+            for (int s = 0; s < 6; ++s) tp[NF][s] = (s == 2) ? W[NF][2] : lds<TC>(sc + own + (s - 2));
+            face_flux2<ORDER, 0, NF>(tp, fmaxf(ax_c, A0[(ty + 1) * TL::AW + tx + 2]), eos, Gx);
         }
         {   // y+ face: cells j-2 .. j+3
-            float tp[6][6];
+            float tp[NW][6];
             const TC *qb = qc + own;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) {
+            for (int f = 0; f < NF; ++f) {
 #pragma unroll
                 for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = (s == 2) ? W[5][2] : lds<TC>(sc + own + (s - 2) * TL::BX);
-            face_flux2<ORDER, 1>(tp, fmaxf(ay_c, A1[(ty + 2) * TL::AW + tx + 1]), gm1, Gy);
+            for (int s = 0; s < 6; ++s) tp[NF][s] = (s == 2) ? W[NF][2] : lds<TC>(sc + own + (s - 2) * TL::BX);
+            face_flux2<ORDER, 1, NF>(tp, fmaxf(ay_c, A1[(ty + 2) * TL::AW + tx + 1]), eos, Gy);
 #pragma unroll
-            for (int c = 0; c < 5; ++c) FY[(c * TY + ty) * TX + tx] = Gy[c];
+            for (int c = 0; c < NC; ++c) FY[(c * TY + ty) * TX + tx] = Gy[c];
         }
         if (warp == 2 % TY && tx < TY) {
             // faces on the tile's low-x edge: between box columns HX-1 | HX of row tx
-            float tp[6][6], Ge[5];
+            float tp[NW][6], Ge[NC];
             const TC *qb = qc + (3 + tx) * TL::BX + TL::HX - 1;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) {
+            for (int f = 0; f < NF; ++f) {
 #pragma unroll
                 for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2));
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = lds<TC>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
-            face_flux2<ORDER, 0>(tp, fmaxf(A0[(tx + 1) * TL::AW + 0], A0[(tx + 1) * TL::AW + 1]), gm1, Ge);
+            for (int s = 0; s < 6; ++s) tp[NF][s] = lds<TC>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
+            face_flux2<ORDER, 0, NF>(tp, fmaxf(A0[(tx + 1) * TL::AW + 0], A0[(tx + 1) * TL::AW + 1]), eos, Ge);
 #pragma unroll
-            for (int c = 0; c < 5; ++c) EX[c * TY + tx] = Ge[c];
+            for (int c = 0; c < NC; ++c) EX[c * TY + tx] = Ge[c];
         }
         if (warp == 3 % TY) {
             // faces on the tile's low-y edge: between box rows 2 | 3 of column tx
-            float tp[6][6], Ge[5];
+            float tp[NW][6], Ge[NC];
             const TC *qb = qc + 2 * TL::BX + TL::HX + tx;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) {
+            for (int f = 0; f < NF; ++f) {
 #pragma unroll
                 for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
             }
 #pragma unroll
-            for (int s = 0; s < 6; ++s) tp[5][s] = lds<TC>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
-            face_flux2<ORDER, 1>(tp, fmaxf(A1[0 * TL::AW + tx + 1], A1[1 * TL::AW + tx + 1]), gm1, Ge);
+            for (int s = 0; s < 6; ++s) tp[NF][s] = lds<TC>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
+            face_flux2<ORDER, 1, NF>(tp, fmaxf(A1[0 * TL::AW + tx + 1], A1[1 * TL::AW + tx + 1]), eos, Ge);
 #pragma unroll
-            for (int c = 0; c < 5; ++c) EY[c * TX + tx] = Ge[c];
+            for (int c = 0; c < NC; ++c) EY[c * TX + tx] = Ge[c];
         }
         __syncthreads();                                   // the only barrier of the step
         if (tid == 0 && t + 3 + TL::NSLOT < n_planes) {              // slot of plane pc is free again
@@ -386,11 +436,11 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         }
 
         // z+ face (cells k-2 .. k+3 of the own column), then the divergence
-        float Gz[5];
-        face_flux2<ORDER, 2>(W, fmaxf(az_c, az_n), gm1, Gz);
-        float r[5];
+        float Gz[NC];
+        face_flux2<ORDER, 2, NF>(W, fmaxf(az_c, az_n), eos, Gz);
+        float r[NC];
 #pragma unroll
-        for (int c = 0; c < 5; ++c) {
+        for (int c = 0; c < NC; ++c) {
             float gxm = __shfl_up_sync(0xffffffffu, Gx[c], 1);
             if (tx == 0) gxm = EX[c * TY + ty];
             const float gym = (ty == 0) ? EY[c * TX + tx] : FY[(c * TY + ty - 1) * TX + tx];
@@ -401,14 +451,16 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             r[c] = __fmul_rn(-hdx, acc);
             Gz_prev[c] = Gz[c];
         }
+        // two fluids: + a1 div u with the face velocities u^ (r[NF] = -(1/dx) sum_d (u^+ - u^-))
+        if (TWO) r[NF - 1] = __fmaf_rn(-W[NF - 1][2], r[NF], r[NF - 1]);
         if (valid) {
             if (!FUSE) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) a.r[c][id] = r[c];
+                for (int c = 0; c < NF; ++c) a.r[c][id] = r[c];
             } else {
-                float o[5];
+                float o[NF];
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
+                for (int c = 0; c < NF; ++c) {
                     const float qs = W[c][2];
                     const float qn = a.read_qn ? qn_pre[c] : qs;
                     o[c] = __fmaf_rn(a.beta, __fmaf_rn(a.dt, r[c], __fsub_rn(qs, qn)), qn);
@@ -417,15 +469,16 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
                 if (a.wave && kz0 + t >= g.wk0 && kz0 + t < g.wk1) {
                     if (sizeof(T) < 4) {
 #pragma unroll
-                        for (int c = 0; c < 5; ++c) o[c] = ldf(reinterpret_cast<const T *>(a.qout[c]) + id);
+                        for (int c = 0; c < NF; ++c) o[c] = ldf(reinterpret_cast<const T *>(a.qout[c]) + id);
                     }
-                    vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], a.gamma, bad));
+                    if (TWO) vmax = fmaxf(vmax, wavespeed_of2(o, eos.k1, eos.k2, bad));
+                    else vmax = fmaxf(vmax, wavespeed_of(o[0], o[1], o[2], o[3], o[4], a.gamma, bad));
                 }
             }
         }
         // slide the window
 #pragma unroll
-        for (int f = 0; f < 6; ++f) {
+        for (int f = 0; f < NW; ++f) {
 #pragma unroll
             for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];
         }
@@ -473,7 +526,7 @@ int rhs_tile_default_zc(const Grid &g)
 }
 
 int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
-                       RhsTileMaps *out, const char **err)
+                       int nf, RhsTileMaps *out, const char **err)
 {
     out->valid = false;
     if (!igr_tma::get_encode()) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
@@ -484,9 +537,9 @@ int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_
     for (int b = 0; b < 3; ++b) {
         const StagePtrs &s = st[b < n_state ? b : n_state - 1];
         const cuuint64_t fstride = (cuuint64_t)((char *)s.f[1] - (char *)s.f[0]);
-        cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 5 };
+        cuuint64_t dims[4] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, (cuuint64_t)nf };
         cuuint64_t strides[3] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es, fstride };
-        cuuint32_t box[4] = { bx, by, 1, 5 };
+        cuuint32_t box[4] = { bx, by, 1, (cuuint32_t)nf };
         if (!igr_tma::encode(&out->q[b], dt, 4, s.f[0], dims, strides, box)) { *err = "cuTensorMapEncodeTiled(q) failed"; return 2; }
     }
     for (int b = 0; b < 2; ++b) {
@@ -501,17 +554,17 @@ int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_
 
 namespace {
 
-template <typename T, int TY, int ORDER, bool FUSE>
+template <typename T, int TY, int ORDER, bool FUSE, int NF = 5>
 void launch_one(const Grid &g, const CUtensorMap &qmap, const CUtensorMap &smap, RhsTileArgs a, cudaStream_t st)
 {
-    using TL = Tile<T, TY>;
+    using TL = Tile<T, TY, NF>;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_rhs_tile<T, TY, ORDER, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, TL::TOTAL);
+        cudaFuncSetAttribute(k_rhs_tile<T, TY, ORDER, FUSE, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, TL::TOTAL);
         configured = true;
     }
     dim3 grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + a.zc - 1) / a.zc);
-    k_rhs_tile<T, TY, ORDER, FUSE><<<grid, TX * TY, TL::TOTAL, st>>>(qmap, smap, g, a);
+    k_rhs_tile<T, TY, ORDER, FUSE, NF><<<grid, TX * TY, TL::TOTAL, st>>>(qmap, smap, g, a);
 }
 
 template <typename T>
@@ -536,6 +589,12 @@ void launch_rhs_tile(const Grid &g, int storage, int order, bool fused, const CU
                      const CUtensorMap &smap, RhsTileArgs a, cudaStream_t st)
 {
     if (a.zc <= 0) a.zc = rhs_tile_default_zc(g);
+    if (a.nf == 7) {
+        // two fluids (NEXT-3): fp32 storage, order 5, 32 x 8 tiles (igr_create_ex refuses the other combinations)
+        if (fused) launch_one<float, 8, 5, true, 7>(g, qmap, smap, a, st);
+        else launch_one<float, 8, 5, false, 7>(g, qmap, smap, a, st);
+        return;
+    }
     if (storage == 0) launch_t<float>(g, order, fused, qmap, smap, a, st);
     else if (storage == 1) launch_t<__half>(g, order, fused, qmap, smap, a, st);
     else launch_t<__nv_bfloat16>(g, order, fused, qmap, smap, a, st);

@@ -37,7 +37,7 @@ class IgrError(RuntimeError):
 
 
 class Patch(C.Structure):
-    _fields_ = [(n, C.c_double) for n in ("c0", "c1", "radius", "edge", "rho", "u", "v", "w", "p")]
+    _fields_ = [(n, C.c_double) for n in ("c0", "c1", "radius", "edge", "rho", "u", "v", "w", "p", "a1", "rho2")]
 
 
 class BC(C.Structure):
@@ -47,8 +47,8 @@ class BC(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("storage", C.c_int32), ("fused", C.c_int32), ("variant", C.c_int32),
-                ("reserved", C.c_int32), ("stream", C.c_void_p),
-                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+                ("n_fluids", C.c_int32), ("stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("gamma2", C.c_double)]
 
 
 class Export(C.Structure):
@@ -107,14 +107,15 @@ def lib():
 
 
 def make_bc(faces, patches=None):
-    """faces: 6 codes (x-,x+,y-,y+,z-,z+); patches: {face: [(c0,c1,radius,edge,rho,u,v,w,p), ...]}"""
+    """faces: 6 codes (x-,x+,y-,y+,z-,z+); patches: {face: [(c0,c1,radius,edge,rho,u,v,w,p[,a1,rho2]), ...]}
+    (a1, rho2: two fluids only, igr.h igr_patch; default 1, 0)."""
     bc, keep = BC(), []
     for f in range(6):
         bc.face[f] = int(faces[f])
         plist = (patches or {}).get(f, [])
         bc.n_patches[f] = len(plist)
         if plist:
-            arr = (Patch * len(plist))(*[Patch(*map(float, p)) for p in plist])
+            arr = (Patch * len(plist))(*[Patch(*map(float, tuple(p) + (1.0, 0.0)[len(p) - 9:])) for p in plist])
             keep.append(arr)
             bc.patches[f] = C.cast(arr, C.POINTER(Patch))
     return bc, keep
@@ -152,14 +153,17 @@ class Solver:
     """igr_create_ex / igr_destroy and the calls of include/igr.h on one solver object."""
 
     def __init__(self, nx, ny, nz, dx, gamma, alpha, order=5, n_jacobi=5, faces=(0,) * 6, patches=None,
-                 storage=STORE_F32, fused=1, variant=VARIANT_TILED, device="cuda:0", own_workspace=True):
+                 storage=STORE_F32, fused=1, variant=VARIANT_TILED, device="cuda:0", own_workspace=True,
+                 n_fluids=1, gamma2=0.0):
         L = lib()
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)
+        self.nf = 7 if n_fluids == 2 else 5          # fields of "the state" (igr.h, igr_options.n_fluids)
         self.device = torch.device(device)
         self._h = None
         opt = Options()
         opt.storage, opt.fused, opt.variant = storage, fused, variant
+        opt.n_fluids, opt.gamma2 = n_fluids, gamma2
         if not torch.cuda.is_available():
             raise IgrError(ERR_CUDA, "no CUDA device: libigr has no CPU fallback")
         torch.cuda.set_device(self.device)
@@ -180,6 +184,8 @@ class Solver:
 
     @classmethod
     def for_workload(cls, w, **kw):
+        if getattr(w, "gamma2", 0.0):
+            kw = dict(n_fluids=2, gamma2=w.gamma2, **kw)
         return cls(w.nx, w.ny, w.nz, w.dx, w.gamma, w.alpha, order=w.order, n_jacobi=w.n_jacobi,
                    faces=w.faces, patches=w.patches, **kw)
 
@@ -200,21 +206,22 @@ class Solver:
 
     # ---- igr.h calls
     def set_state(self, q):
-        self._check(lib().igr_set_state(self._h, _addr(q, (5,) + self.shape)))
+        self._check(lib().igr_set_state(self._h, _addr(q, (self.nf,) + self.shape)))
 
     def get_state(self, out=None):
-        out = np.empty((5,) + self.shape, np.float32) if out is None else out
-        self._check(lib().igr_get_state(self._h, _addr(out, (5,) + self.shape, True)))
+        out = np.empty((self.nf,) + self.shape, np.float32) if out is None else out
+        self._check(lib().igr_get_state(self._h, _addr(out, (self.nf,) + self.shape, True)))
         return out
 
     def set_state_planes(self, k0, q):
         """q: [5][nk][ny][nx], planes k0 .. k0 + nk - 1 (Sigma is left as it is)."""
         nk = int(q.shape[1])
-        self._check(lib().igr_set_state_planes(self._h, int(k0), nk, _addr(q, (5, nk, self.ny, self.nx))))
+        self._check(lib().igr_set_state_planes(self._h, int(k0), nk, _addr(q, (self.nf, nk, self.ny, self.nx))))
 
     def get_state_planes(self, k0, nk, out=None):
-        out = np.empty((5, nk, self.ny, self.nx), np.float32) if out is None else out
-        self._check(lib().igr_get_state_planes(self._h, int(k0), int(nk), _addr(out, (5, nk, self.ny, self.nx), True)))
+        out = np.empty((self.nf, nk, self.ny, self.nx), np.float32) if out is None else out
+        self._check(lib().igr_get_state_planes(self._h, int(k0), int(nk),
+                                               _addr(out, (self.nf, nk, self.ny, self.nx), True)))
         return out
 
     def set_sigma(self, f):

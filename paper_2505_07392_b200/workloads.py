@@ -40,10 +40,15 @@ class Workload:
     global_shape: tuple = None    # (nx,ny,nz) of the full domain the noise is indexed on
     kind: str = ""
     params: dict = field(default_factory=dict)
+    gamma2: float = 0.0           # > 1: the two-fluid variant (NEXT-3, reading A21): `gamma` is fluid 1's exponent
 
     @property
     def n_cells(self):
         return self.nx * self.ny * self.nz
+
+    @property
+    def nf(self):                 # fields of the conserved state
+        return 7 if self.gamma2 else 5
 
 
 # --------------------------------------------------------------------------- noise
@@ -86,6 +91,21 @@ def _conserved(w, rho, u, v, ww, p, out_dtype, nk):
     return q
 
 
+def _conserved2(w, a1, rho1, rho2, u, v, ww, p, out_dtype, nk):
+    """Two fluids (reading A21): (a1, rho1, rho2, u, p) -> (a1 rho1, a2 rho2, rho u, E, a1) with the isobaric
+    mixture rule E = p Gamma + rho |u|^2 / 2, Gamma = a1/(gamma1 - 1) + (1 - a1)/(gamma2 - 1)."""
+    shape = (nk, w.ny, w.nx)
+    a1, rho1, rho2, u, v, ww, p = (torch.broadcast_to(t, shape) for t in (a1, rho1, rho2, u, v, ww, p))
+    q = torch.empty((7,) + shape, dtype=out_dtype, device=a1.device)
+    m1, m2 = a1 * rho1, (1.0 - a1) * rho2
+    rho = m1 + m2
+    q[0], q[1] = m1, m2
+    q[2], q[3], q[4] = rho * u, rho * v, rho * ww
+    q[5] = p * (a1 / (w.gamma - 1.0) + (1.0 - a1) / (w.gamma2 - 1.0)) + 0.5 * rho * (u * u + v * v + ww * ww)
+    q[6] = a1
+    return q
+
+
 def state(w, device="cpu", dtype=torch.float32, slab=None):
     """Initial conserved state of workload `w`, [5][nz][ny][nx], generated on `device` (in z-slabs
     so that the fp64 temporaries of the large cases stay small)."""
@@ -93,7 +113,7 @@ def state(w, device="cpu", dtype=torch.float32, slab=None):
         slab = max(1, min(w.nz, (1 << 24) // (w.nx * w.ny) or 1))
     if slab >= w.nz:
         return _state_slab(w, device, dtype, 0, w.nz)
-    q = torch.empty((5, w.nz, w.ny, w.nx), dtype=dtype, device=torch.device(device))
+    q = torch.empty((w.nf, w.nz, w.ny, w.nx), dtype=dtype, device=torch.device(device))
     for k0 in range(0, w.nz, slab):
         nk = min(slab, w.nz - k0)
         q[:, k0:k0 + nk] = _state_slab(w, device, dtype, k0, nk)
@@ -162,7 +182,21 @@ def _state_slab(w, device, dtype, kz0, nk):
         u = amp * hash_noise(gi, gj, gk, gshape, 1, seed)
         v = amp * hash_noise(gi, gj, gk, gshape, 2, seed)
         ww = amp * hash_noise(gi, gj, gk, gshape, 3, seed) + w_j * s
+        if w.gamma2:
+            # two fluids: the jet gas is fluid 1 (gamma), the gas at rest fluid 2 (gamma2); the volume fraction
+            # follows the same profile s, kept inside (eps, 1 - eps) so that both partial densities stay positive
+            eps = P.get("a1_floor", 1e-3)
+            a1 = eps + (1.0 - 2.0 * eps) * s
+            return _conserved2(w, a1, rho_j * one, 1.0 * one, u, v, ww, p, dtype, nk)
         return _conserved(w, rho, u, v, ww, p, dtype, nk)
+    if w.kind == "two_fluid_vortex":
+        # smooth periodic two-fluid test state: Taylor-Green-like velocity at Mach ~0.5, a smooth blob of fluid 1
+        a1 = 0.5 + 0.4 * torch.sin(x) * torch.sin(y) * torch.cos(z)
+        u = 0.5 * torch.sin(x) * torch.cos(y) * torch.cos(z) + 0.2
+        v = -0.5 * torch.cos(x) * torch.sin(y) * torch.cos(z) - 0.1
+        ww = 0.3 * torch.sin(z) * torch.cos(x)
+        p = 1.0 + 0.1 * (torch.cos(2 * x) + torch.cos(2 * y)) * (torch.cos(2 * z) + 2.0) / 4.0
+        return _conserved2(w, a1, 1.0 * one, 0.3 * one, u, v, ww, p, dtype, nk)
     if w.kind == "uniform":
         return _conserved(w, P["rho"] * one, P["u"] * one, P["v"] * one, P["w"] * one,
                           P["p"] * one, dtype, nk)
@@ -235,6 +269,22 @@ def jets33(n=1024, n_steps=100, radius=8, rings=((14, 3), (44, 10), (84, 20)), n
                     params={"noise": noise, "seed": seed, "stub_delta": stub_delta,
                             "jet_centers": [(cx, cy, radius) for cx, cy in centers],
                             "jet_state": (0.5, 3.0 * math.sqrt(1.4 * 3.0 / 0.5), 3.0)})
+
+
+def two_fluid_vortex(n=32, gamma1=1.4, gamma2=1.67):
+    """Smooth periodic two-fluid state on [0, 2 pi]^3 (parity tests of the two-fluid variant)."""
+    dx = 2.0 * math.pi / n
+    return Workload("two_fluid_vortex_%d" % n, n, n, n, dx, gamma=gamma1, alpha=10 * dx * dx, kind="two_fluid_vortex",
+                    gamma2=gamma2)
+
+
+def two_fluid(w, gamma1=1.3, gamma2=1.4, a1_floor=1e-3):
+    """The two-fluid variant of a jets workload (the paper's timed problem is a two-fluid jet, L274): the jet gas
+    is fluid 1 (gamma1), the gas at rest fluid 2 (gamma2); the patches carry (a1, rho2) = (1 - a1_floor, 1)."""
+    assert w.kind == "jets"
+    patches = {f: [tuple(p[:9]) + (1.0 - a1_floor, 1.0) for p in pl] for f, pl in w.patches.items()}
+    return replace(w, name=w.name.replace("jets", "jets2f"), gamma=gamma1, gamma2=gamma2, patches=patches,
+                   params={**w.params, "a1_floor": a1_floor})
 
 
 def uniform(nx, ny, nz, dx, rho, u, v, w, p, faces=(0, 0, 0, 0, 0, 0), patches=None):

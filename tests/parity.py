@@ -11,7 +11,12 @@ def norms(got, ref):
     """Per-field (max-rel, L1-rel); the three momentum components share one denominator."""
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
-    groups = [[0], [1, 2, 3], [4]] if ref.shape[0] == 5 else [[c] for c in range(ref.shape[0])]
+    if ref.shape[0] == 5:
+        groups = [[0], [1, 2, 3], [4]]
+    elif ref.shape[0] == 7:                       # two fluids: (a1 rho1, a2 rho2, m, E, a1)
+        groups = [[0], [1], [2, 3, 4], [5], [6]]
+    else:
+        groups = [[c] for c in range(ref.shape[0])]
     out = {}
     for grp in groups:
         d = np.abs(got[grp] - ref[grp])
@@ -32,6 +37,11 @@ def scalar_norms(got, ref, floor=0.0):
 
 
 def oracle_for(w, storage=R.STORE_F64):
+    if getattr(w, "gamma2", 0.0):                 # two fluids (igr_ref2.c): patches (.., a1 rho1, a2 rho2, a1, u, v, w, p)
+        patches = {f: [tuple(p[:4]) + (p[9] * p[4], (1.0 - p[9]) * p[10], p[9]) + tuple(p[5:9]) for p in pl]
+                   for f, pl in w.patches.items()}
+        return R.RefSolver2(w.nx, w.ny, w.nz, w.dx, w.gamma, w.gamma2, w.alpha, order=w.order, n_jacobi=w.n_jacobi,
+                            faces=w.faces, patches=patches)
     return R.RefSolver(w.nx, w.ny, w.nz, w.dx, w.gamma, w.alpha, order=w.order, n_jacobi=w.n_jacobi,
                        faces=w.faces, patches=w.patches, storage=storage)
 
