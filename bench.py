@@ -10,7 +10,7 @@ metric = grind time ns/(cell*eqn*RHS) = t_step / (cells * 5 * 3); lower is bette
 Multi-GPU (--gpus N under torchrun, one rank per GPU): weak scaling by z slabs: the
 job is the workload stacked N times along z, every rank owns one copy's planes plus n_jacobi + 3 overlap planes per
 neighbour and pulls its halo planes from the neighbours after every RK stage (CUDA IPC peer copies, or
-torch.distributed send/recv); value = time / (total OWNED cells * 15), time = max over ranks.
+torch.distributed send/recv); value = time / (total OWNED cells * equations * 3), time = max over ranks.
 """
 import argparse
 import json
@@ -57,6 +57,8 @@ def make_workload(name):
     from paper_2505_07392_b200 import workloads as W
     kind, n = name.rsplit("_", 1)
     n = int(n)
+    if kind in ("jets2f33", "jets2f9"):          # two-fluid variant (NEXT-3): the same jets, 7 equations
+        return W.two_fluid(make_workload(kind.replace("2f", "") + "_%d" % n))
     if kind == "jets33":
         scale = n / 1024.0
         if n >= 1024:
@@ -125,8 +127,14 @@ def cpu_baseline(w, n_box=96, steps=2):
     else:
         wb = type(w)(**{**w.__dict__, "nx": min(n_box, w.nx), "ny": min(n_box, w.ny), "nz": min(n_box, w.nz)})
     q = W.state(wb).numpy().astype(np.float64)
-    s = R.RefSolver(wb.nx, wb.ny, wb.nz, wb.dx, wb.gamma, wb.alpha, order=wb.order, n_jacobi=wb.n_jacobi,
-                    faces=wb.faces, patches=wb.patches)
+    if wb.gamma2:        # two fluids: oracle/igr_ref2.c, patches (c0, c1, radius, edge, a1 rho1, a2 rho2, a1, u, v, w, p)
+        pt = {f: [tuple(p[:4]) + (p[9] * p[4], (1.0 - p[9]) * p[10], p[9]) + tuple(p[5:9]) for p in pl]
+              for f, pl in wb.patches.items()}
+        s = R.RefSolver2(wb.nx, wb.ny, wb.nz, wb.dx, wb.gamma, wb.gamma2, wb.alpha, order=wb.order,
+                         n_jacobi=wb.n_jacobi, faces=wb.faces, patches=pt)
+    else:
+        s = R.RefSolver(wb.nx, wb.ny, wb.nz, wb.dx, wb.gamma, wb.alpha, order=wb.order, n_jacobi=wb.n_jacobi,
+                        faces=wb.faces, patches=wb.patches)
     s.set_state(q)
     dt = wb.cfl * wb.dx / s.max_wavespeed()
     s.step(dt)                                   # untimed first touch
@@ -135,17 +143,21 @@ def cpu_baseline(w, n_box=96, steps=2):
         s.step(wb.cfl * wb.dx / s.max_wavespeed())
     dt_wall = time.perf_counter() - t0
     cells = wb.nx * wb.ny * wb.nz
-    return {"value": dt_wall / steps / (cells * 15) * 1e9, "unit": UNIT, "cores": int(os.environ["OMP_NUM_THREADS"]),
+    return {"value": dt_wall / steps / (cells * wb.nf * 3) * 1e9, "unit": UNIT, "cores": int(os.environ["OMP_NUM_THREADS"]),
             "kind": "oracle", "sample": "%dx%dx%d sub-box of %s on the inflow plane, %d steps, fp64, OpenMP"
             % (wb.nx, wb.ny, wb.nz, w.name, steps), "ms_per_step": dt_wall / steps * 1e3}
 
 
-def alg_bytes(row, storage, fused=1):
+def alg_bytes(row, storage, fused=1, nf=5):
     """Algorithmic HBM bytes per cell per launch, averaged over the three stages:
     q and Sigma in the storage type (s bytes), b and r in fp32.  source: 4 q reads + b write; jacobi
     (5 sweeps blocked): rho + b + Sigma in + Sigma out; rhs: 5 q + Sigma reads, then either 5 r writes
     (unfused) or the fused update: q_n reads in stages 2, 3 and 5 q writes; rk_update (unfused only)."""
     s = 4 if storage == "f32" else 2
+    if nf == 7:         # two fluids, fp32, fused: source reads 5 fields and writes b and the mixture density (which
+        #                 is then read with its ghosts); jacobi reads that density; rhs moves 7 fields and Sigma
+        return {"sigma_source": 5 * 4 + 4 + 2 * 4, "jacobi": 16, "rhs": 8 * 4 + 7 * 4 + 2 * 7 * 4 / 3.0,
+                "rk_update": 0.0}[row]
     rhs = 6 * s + (5 * s + 2 * 5 * s / 3.0 if fused else 20)
     return {"sigma_source": 4 * s + 4, "jacobi": 3 * s + 4, "rhs": rhs,
             "rk_update": (5 * (s + 4 + s) + 2 * 5 * (2 * s + 4 + s)) / 3.0}[row]
@@ -195,11 +207,12 @@ def reduce_max(value, world, device="cpu"):
     return float(t.item())
 
 
-def job_numbers(ms_step, cells_per_rank, world):
+def job_numbers(ms_step, cells_per_rank, world, neq=5):
     """Whole-job metric of `world` ranks that each advance `cells_per_rank` owned cells in ms_step (max
-    over ranks): grind time per (cell*eqn*RHS) of the job and aggregate cell updates per second."""
+    over ranks): grind time per (cell*eqn*RHS) of the job (neq equations, 3 RHS evaluations per step) and
+    aggregate cell updates per second."""
     total = cells_per_rank * world
-    return {"grind_ns": ms_step * 1e6 / (total * 15), "cell_updates_per_s": total / (ms_step * 1e-3)}
+    return {"grind_ns": ms_step * 1e6 / (total * neq * 3), "cell_updates_per_s": total / (ms_step * 1e-3)}
 
 
 def run_ours(args):
@@ -236,7 +249,7 @@ def run_ours(args):
         g = igr.Solver.for_workload(w, storage=storage, fused=args.fused, device=dev)
         # the fp32 copy of the initial state stays on the device for restarts only if it fits beside the solver
         free_b = torch.cuda.mem_get_info(torch.device(dev))[0]
-        q0 = W.state(w, device=dev) if free_b > 5 * cells * 4 + (12 << 30) else None
+        q0 = W.state(w, device=dev) if free_b > w.nf * cells * 4 + (12 << 30) else None
     if args.mu > 0 or args.zeta > 0:
         g.set_viscosity(args.mu, args.zeta)
     filled = [False]
@@ -307,7 +320,7 @@ def run_ours(args):
     clocks = sampler.stop()
     ms = reduce_max(ms, world, rdev)
     ms_step = ms / args.steps
-    job = job_numbers(ms_step, cells, world)
+    job = job_numbers(ms_step, cells, world, w.nf)
     grind = job["grind_ns"]
 
     # per-row CUDA-event timing on the solver's stream (separate region, same state)
@@ -334,7 +347,7 @@ def run_ours(args):
     dom = max(("sigma_source", "jacobi", "rhs", "rk_update"), key=lambda r: rows[r][0])
     peak, peak_src = measured_peaks()
     main_rows = [r for r in ("sigma_source", "jacobi", "rhs", "rk_update") if row_ms[r] > 0]
-    hbm_gbs = {r: alg_bytes(r, args.storage, args.fused) * cells / (row_ms[r] * 1e-3) / 1e9 for r in main_rows}
+    hbm_gbs = {r: alg_bytes(r, args.storage, args.fused, w.nf) * cells / (row_ms[r] * 1e-3) / 1e9 for r in main_rows}
     alu_tf = {r: ALG_FLOP[r] * cells / (row_ms[r] * 1e-3) / 1e12 for r in main_rows}
     alu_peak = alu_peak_tflops()
     # the dominant kernel is reported against the roofline that binds it: the larger of the two fractions
@@ -351,14 +364,14 @@ def run_ours(args):
         "traffic": traffic,
         "traffic_unit": ("bytes per launch, mean of the captured stages %s (ncu --set full, profiles/dram_traffic.csv)"
                          % traffic_stages) if traffic else "no ncu capture of this workload / storage in profiles/",
-        "alg_bytes_per_cell": alg_bytes(dom, args.storage, args.fused),
+        "alg_bytes_per_cell": alg_bytes(dom, args.storage, args.fused, w.nf),
         "hbm": {"achieved_gbs": hbm_gbs[dom], "peak_gbs": peak, "frac": hbm_gbs[dom] / peak, "peak_source": peak_src,
                 "frac_of_nominal_8tbs": hbm_gbs[dom] / 8000.0},
         "avg_launch_ms": row_ms[dom], "share_of_step": rows[dom][0] / nprof / step_ms_prof,
         "rows_ms_per_call": row_ms,
         "rows_hbm_frac": {r: hbm_gbs[r] / peak for r in main_rows},
         "rows_alu_frac": {r: alu_tf[r] / alu_peak for r in main_rows},
-        "step_hbm_frac": sum(3 * alg_bytes(r, args.storage, args.fused) for r in main_rows) * cells
+        "step_hbm_frac": sum(3 * alg_bytes(r, args.storage, args.fused, w.nf) for r in main_rows) * cells
         / (ms_step * 1e-3) / 1e9 / peak})
 
     # end to end through the C ABI with HOST buffers: set_state (H2D) + wave speed + step + get_state (D2H)
@@ -366,10 +379,10 @@ def run_ours(args):
     if args.e2e_steps > 0:
         lw = ss.slab.local if ss else w      # the arrays the rank's C-ABI calls move (extended slab)
         try:
-            host = torch.empty((5, lw.nz, lw.ny, lw.nx), dtype=torch.float32, pin_memory=True)
+            host = torch.empty((w.nf, lw.nz, lw.ny, lw.nx), dtype=torch.float32, pin_memory=True)
             pinned = True
         except RuntimeError:
-            host = torch.empty((5, lw.nz, lw.ny, lw.nx), dtype=torch.float32)
+            host = torch.empty((w.nf, lw.nz, lw.ny, lw.nx), dtype=torch.float32)
             pinned = False
         load_initial()                           # a fresh state: the e2e steps never meet a reset
         g.get_state(host)
@@ -384,15 +397,15 @@ def run_ours(args):
         barrier()
         t_e2e = (time.perf_counter() - t0) / args.e2e_steps
         t_e2e = reduce_max(t_e2e, world, rdev)
-        nbytes = 5 * lw.n_cells * 4
-        e2e = {"value": job_numbers(t_e2e * 1e3, cells, world)["grind_ns"], "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        nbytes = w.nf * lw.n_cells * 4
+        e2e = {"value": job_numbers(t_e2e * 1e3, cells, world, w.nf)["grind_ns"], "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 8, "ms_per_step": t_e2e * 1e3, "pinned_host": pinned}
 
     out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "storage_dtype": args.storage, "data": "synthetic",
            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
-                      "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
+                      "equations": w.nf, "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
                       "cfl": w.cfl,
                       "parallelism": ("z slabs: %d ranks x %d owned planes + %d overlap planes per neighbour, one halo "
                                       "exchange per RK stage (%s)" % (world, w.nz, ss.slab.overlap, ss.exchange_kind))
