@@ -501,6 +501,9 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 // ======================================================================================= host
 namespace {
 
+// two fluids: 168 registers per thread, one CTA per SM: 12 rows (384 threads) fill the register file
+constexpr int TY2 = 12;
+
 int tile_ty(const Grid &g)
 {
     static int force = -1;                       // IGR_RHS_TY=8|16 overrides the heuristic (tuning)
@@ -532,7 +535,7 @@ int rhs_tile_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_
     if (!igr_tma::get_encode()) { *err = "cuTensorMapEncodeTiled entry point not available"; return 1; }
     const size_t es = storage == 0 ? 4 : 2;
     const CUtensorMapDataType dt = igr_tma::data_type(storage);
-    const int hx = 16 / (int)es, ty = tile_ty(g);
+    const int hx = 16 / (int)es, ty = nf == 7 ? TY2 : tile_ty(g);
     const cuuint32_t bx = TX + 2 * hx, by = ty + 6;
     for (int b = 0; b < 3; ++b) {
         const StagePtrs &s = st[b < n_state ? b : n_state - 1];
@@ -591,8 +594,8 @@ void launch_rhs_tile(const Grid &g, int storage, int order, bool fused, const CU
     if (a.zc <= 0) a.zc = rhs_tile_default_zc(g);
     if (a.nf == 7) {
         // two fluids (NEXT-3): fp32 storage, order 5, 32 x 8 tiles (igr_create_ex refuses the other combinations)
-        if (fused) launch_one<float, 8, 5, true, 7>(g, qmap, smap, a, st);
-        else launch_one<float, 8, 5, false, 7>(g, qmap, smap, a, st);
+        if (fused) launch_one<float, TY2, 5, true, 7>(g, qmap, smap, a, st);
+        else launch_one<float, TY2, 5, false, 7>(g, qmap, smap, a, st);
         return;
     }
     if (storage == 0) launch_t<float>(g, order, fused, qmap, smap, a, st);
