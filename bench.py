@@ -34,7 +34,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="jets33_1024")
-    ap.add_argument("--storage", default="f32", choices=["f32", "f16", "bf16"])
+    ap.add_argument("--storage", default="f32", choices=["f32", "f16", "bf16", "f64"],
+                    help="f16 / bf16: reduced-precision storage, fp32 arithmetic (L264); f64: fp64 storage AND arithmetic "
+                         "(NEXT-4: one thread per cell, for the paper's FP64 column)")
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -153,6 +155,9 @@ def alg_bytes(row, storage, fused=1, nf=5):
     q and Sigma in the storage type (s bytes), b and r in fp32.  source: 4 q reads + b write; jacobi
     (5 sweeps blocked): rho + b + Sigma in + Sigma out; rhs: 5 q + Sigma reads, then either 5 r writes
     (unfused) or the fused update: q_n reads in stages 2, 3 and 5 q writes; rk_update (unfused only)."""
+    if storage == "f64":    # fp64 mode: every field 8 bytes, one launch per Jacobi sweep, unfused update
+        return {"sigma_source": 4 * 8 + 8, "jacobi": 5 * 4 * 8, "rhs": 6 * 8 + 5 * 8,
+                "rk_update": (5 * 24 + 2 * 5 * 32) / 3.0}[row]
     s = 4 if storage == "f32" else 2
     if nf == 7:         # two fluids, fp32, fused: source reads 5 fields and writes b and the mixture density (which
         #                 is then read with its ghosts); jacobi reads that density; rhs moves 7 fields and Sigma
@@ -233,7 +238,9 @@ def run_ours(args):
             dist.init_process_group("gloo")
     rdev = dev if args.backend == "nccl" else "cpu"      # where the scalar reductions live
     w = make_workload(args.workload)
-    storage = {"f32": igr.STORE_F32, "f16": igr.STORE_F16, "bf16": igr.STORE_BF16}[args.storage]
+    storage = {"f32": igr.STORE_F32, "f16": igr.STORE_F16, "bf16": igr.STORE_BF16, "f64": igr.STORE_F64}[args.storage]
+    if args.storage == "f64":
+        args.fused = 0                    # the fp64 mode runs one kernel per row
     cells = w.n_cells                     # cells OWNED per rank (weak scaling: the job has world x cells)
     ss = None
     if world > 1:
@@ -403,7 +410,8 @@ def run_ours(args):
 
     out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "storage_dtype": args.storage, "data": "synthetic",
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.storage == "f64" else "f32",
+           "storage_dtype": args.storage, "data": "synthetic",
            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "cells_per_gpu": cells,
                       "equations": w.nf, "storage": args.storage, "fused": args.fused, "mu": args.mu, "zeta": args.zeta, "n_jacobi": w.n_jacobi, "order": w.order,
                       "cfl": w.cfl,

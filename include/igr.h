@@ -56,6 +56,12 @@ typedef enum {
 #define IGR_STORE_F32  0
 #define IGR_STORE_F16  1
 #define IGR_STORE_BF16 2
+/* fp64 MODE: fp64 storage AND fp64 arithmetic, for a like-for-like column beside the paper's
+ * FP64 grind times (Table 1).  One thread per cell, one launch per row and per Jacobi sweep, IEEE
+ * division and square root (parity with the fp64 oracle <= 1e-12).  `fused` and `variant` are ignored; one fluid,
+ * no viscosity, no slabs; igr_get_padded / igr_get_source / igr_set_source / igr_get_rhs are not available.  The
+ * fp32 calls convert at the boundary; igr_set_state_f64 / igr_get_state_f64 / igr_get_sigma_f64 move fp64 arrays. */
+#define IGR_STORE_F64  3
 
 #define IGR_VARIANT_TILED  0
 #define IGR_VARIANT_SIMPLE 1
@@ -137,6 +143,10 @@ int igr_get_state(igr_solver *s, float *q);
  * the middle of a step; IGR_ERR_ARG for a range outside [0, nz). */
 int igr_set_state_planes(igr_solver *s, int k0, int nk, const float *q);
 int igr_get_state_planes(igr_solver *s, int k0, int nk, float *q);
+/* fp64 arrays (IGR_STORE_F64 only, else IGR_ERR_ARG): same layouts, host or device pointers */
+int igr_set_state_f64(igr_solver *s, const double *q);
+int igr_get_state_f64(igr_solver *s, double *q);
+int igr_get_sigma_f64(igr_solver *s, double *f);
 /* Sigma is part of a restart because of the warm start (L130, L138).  f: [nz][ny][nx]. */
 int igr_set_sigma(igr_solver *s, const float *f);
 int igr_get_sigma(igr_solver *s, float *f);

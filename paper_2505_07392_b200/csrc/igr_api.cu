@@ -19,7 +19,7 @@ constexpr size_t kAlign = 256;
 constexpr size_t kStageBytes = 64u << 20;          // staging buffer for host <-> device copies
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-inline size_t elem_size(int storage) { return storage == IGR_STORE_F32 ? 4 : 2; }
+inline size_t elem_size(int storage) { return storage == IGR_STORE_F64 ? 8 : (storage == IGR_STORE_F32 ? 4 : 2); }
 
 Grid make_grid(int nx, int ny, int nz, int storage, const int32_t *faces)
 {
@@ -49,7 +49,7 @@ Layout make_layout(const Grid &g, int storage, int fused, int variant, int nf = 
 {
     Layout L;
     L.q_bytes = align_up((size_t)g.np * elem_size(storage), kAlign);
-    L.f_bytes = align_up((size_t)g.np * 4, kAlign);
+    L.f_bytes = align_up((size_t)g.np * (storage == IGR_STORE_F64 ? 8 : 4), kAlign);   // b, r: fp32 (fp64 mode: fp64)
     L.n_state = fused ? 3 : 2;
     // the fused tiled step never materialises r: it is allocated only if an unfused row, igr_get_rhs or
     // the viscous path asks for it (5 fp32 fields less: 18 instead of 23 fields at rest)
@@ -85,6 +85,7 @@ struct igr_solver {
     WaveResult *wave = nullptr;      // device
     bool wave_valid = false;         // wave holds the wave speed of the current state
     BcDesc bc;
+    Inflow64 bc64;                   // fp64 mode: the same tables in double
     std::vector<void *> bc_allocs;   // device arrays of the inflow faces
     std::string err;
     double mu = 0, zeta = 0;         // viscosity (NEXT-1); 0, 0: inviscid
@@ -133,6 +134,7 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
     for (int f = 0; f < 6; ++f) {
         InflowFace &F = s->bc.inflow[f];
         F.weight = nullptr; F.fixed = nullptr; F.n0 = F.n1 = 0;
+        s->bc64.weight[f] = nullptr; s->bc64.fixed[f] = nullptr; s->bc64.n0[f] = s->bc64.n1[f] = 0;
         if (bc->face[f] != IGR_BC_INFLOW || bc->n_patches[f] <= 0) continue;
         if (!bc->patches[f]) return s->fail(IGR_ERR_ARG, "igr_create: inflow face without patches array");
         const int a = f / 2;
@@ -140,6 +142,8 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
         F.n1 = (a == 2) ? n[1] : n[2];
         const int nf = s->nf;
         std::vector<float> w((size_t)F.n0 * F.n1), fx((size_t)F.n0 * F.n1 * nf, 0.f);
+        std::vector<double> w64, fx64;
+        if (s->storage == IGR_STORE_F64) { w64.assign(w.size(), 0.0); fx64.assign(fx.size(), 0.0); }
         for (int t1 = 0; t1 < F.n1; ++t1)
             for (int t0 = 0; t0 < F.n0; ++t0) {
                 double best = 0.0; const igr_patch *bp = nullptr;
@@ -156,6 +160,7 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
                     const double v[5] = { bp->rho, bp->rho * bp->u, bp->rho * bp->v, bp->rho * bp->w,
                                           bp->p / (s->gamma - 1.0) + ke };
                     for (int c = 0; c < 5; ++c) fx[id * 5 + c] = (float)v[c];
+                    if (!w64.empty()) { w64[id] = best; for (int c = 0; c < 5; ++c) fx64[id * 5 + c] = v[c]; }
                 } else if (bp) {             // two fluids (igr.h, igr_patch): rho = fluid 1, rho2 = fluid 2
                     const double m1 = bp->a1 * bp->rho, m2 = (1.0 - bp->a1) * bp->rho2, rm = m1 + m2;
                     const double ke = 0.5 * rm * (bp->u * bp->u + bp->v * bp->v + bp->w * bp->w);
@@ -171,6 +176,15 @@ int build_inflow(igr_solver *s, const igr_bc *bc)
         IGR_CUDA_OK(cudaMemcpy(dw, w.data(), w.size() * 4, cudaMemcpyHostToDevice));
         IGR_CUDA_OK(cudaMemcpy(dfx, fx.data(), fx.size() * 4, cudaMemcpyHostToDevice));
         F.weight = dw; F.fixed = dfx;
+        if (!w64.empty()) {
+            double *dw64 = nullptr, *dfx64 = nullptr;
+            if (cudaMalloc(&dw64, w64.size() * 8) != cudaSuccess || cudaMalloc(&dfx64, fx64.size() * 8) != cudaSuccess)
+                return s->fail(IGR_ERR_ALLOC, "igr_create: cudaMalloc of inflow tables failed");
+            s->bc_allocs.push_back(dw64); s->bc_allocs.push_back(dfx64);
+            IGR_CUDA_OK(cudaMemcpy(dw64, w64.data(), w64.size() * 8, cudaMemcpyHostToDevice));
+            IGR_CUDA_OK(cudaMemcpy(dfx64, fx64.data(), fx64.size() * 8, cudaMemcpyHostToDevice));
+            s->bc64.weight[f] = dw64; s->bc64.fixed[f] = dfx64; s->bc64.n0[f] = F.n0; s->bc64.n1[f] = F.n1;
+        }
     }
     return IGR_OK;
 }
@@ -184,22 +198,28 @@ bool is_device_pointer(const void *p)
 
 // copy one user field (interior, fp32, host or device) into / out of a padded field
 // (planes [kfirst, kfirst + nplanes) of the field; `user` holds exactly those planes; nplanes < 0: all)
-int field_in(igr_solver *s, const float *user, void *field, int storage, int kfirst = 0, int nplanes = -1)
+// `ubytes`: element size of the user array (4: fp32, the ABI's default; 8: the *_f64 calls of the fp64 mode)
+int field_in(igr_solver *s, const void *user, void *field, int storage, int kfirst = 0, int nplanes = -1, int ubytes = 4)
 {
     const Grid &g = s->g;
     if (nplanes < 0) nplanes = g.nz;
+    auto unpack = [&](const void *src, int k0, int nk) {
+        if (storage == IGR_STORE_F64) launch64_unpack(g, src, ubytes == 4, (double *)field, k0, nk, s->stream);
+        else launch_unpack_field(g, storage, (const float *)src, field, k0, nk, s->stream);
+    };
+    if (storage != IGR_STORE_F64 && ubytes != 4) return s->fail(IGR_ERR_ARG, "fp64 arrays: only with IGR_STORE_F64");
     if (is_device_pointer(user)) {
-        launch_unpack_field(g, storage, user, field, kfirst, nplanes, s->stream);
+        unpack(user, kfirst, nplanes);
         return IGR_OK;
     }
-    const size_t plane = (size_t)g.nx * g.ny * 4;
+    const size_t plane = (size_t)g.nx * g.ny * ubytes;
     int chunk = (int)(kStageBytes / plane);
     if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
     for (int k0 = 0; k0 < nplanes; k0 += chunk) {
         const int nk = (nplanes - k0 < chunk) ? nplanes - k0 : chunk;
-        IGR_CUDA_OK(cudaMemcpyAsync(s->stage, user + (size_t)k0 * g.nx * g.ny, nk * plane,
+        IGR_CUDA_OK(cudaMemcpyAsync(s->stage, (const char *)user + (size_t)k0 * plane, nk * plane,
                                     cudaMemcpyHostToDevice, s->stream));
-        launch_unpack_field(g, storage, s->stage, field, kfirst + k0, nk, s->stream);
+        unpack(s->stage, kfirst + k0, nk);
         // the staging buffer is reused by the next chunk and `user` is borrowed for the duration of the call
         // only (igr.h): the copy must have left the host buffer before this returns
         IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
@@ -207,21 +227,26 @@ int field_in(igr_solver *s, const float *user, void *field, int storage, int kfi
     return IGR_OK;
 }
 
-int field_out(igr_solver *s, const void *field, float *user, int storage, int kfirst = 0, int nplanes = -1)
+int field_out(igr_solver *s, const void *field, void *user, int storage, int kfirst = 0, int nplanes = -1, int ubytes = 4)
 {
     const Grid &g = s->g;
     if (nplanes < 0) nplanes = g.nz;
+    auto pack = [&](void *dst, int k0, int nk) {
+        if (storage == IGR_STORE_F64) launch64_pack(g, (const double *)field, dst, ubytes == 4, k0, nk, s->stream);
+        else launch_pack_field(g, storage, field, (float *)dst, k0, nk, s->stream);
+    };
+    if (storage != IGR_STORE_F64 && ubytes != 4) return s->fail(IGR_ERR_ARG, "fp64 arrays: only with IGR_STORE_F64");
     if (is_device_pointer(user)) {
-        launch_pack_field(g, storage, field, user, kfirst, nplanes, s->stream);
+        pack(user, kfirst, nplanes);
         return IGR_OK;
     }
-    const size_t plane = (size_t)g.nx * g.ny * 4;
+    const size_t plane = (size_t)g.nx * g.ny * ubytes;
     int chunk = (int)(kStageBytes / plane);
     if (chunk < 1) return s->fail(IGR_ERR_ARG, "igr: one z-plane exceeds the staging buffer");
     for (int k0 = 0; k0 < nplanes; k0 += chunk) {
         const int nk = (nplanes - k0 < chunk) ? nplanes - k0 : chunk;
-        launch_pack_field(g, storage, field, s->stage, kfirst + k0, nk, s->stream);
-        IGR_CUDA_OK(cudaMemcpyAsync(user + (size_t)k0 * g.nx * g.ny, s->stage, nk * plane,
+        pack(s->stage, kfirst + k0, nk);
+        IGR_CUDA_OK(cudaMemcpyAsync((char *)user + (size_t)k0 * plane, s->stage, nk * plane,
                                     cudaMemcpyDeviceToHost, s->stream));
         IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
     }
@@ -274,10 +299,11 @@ size_t igr_workspace_bytes(int nx, int ny, int nz, const igr_options *opt)
 {
     if (nx < 1 || ny < 1 || nz < 1) return 0;
     const int storage = opt ? opt->storage : IGR_STORE_F32;
-    const int fused = opt ? opt->fused : 1;
-    if (storage < 0 || storage > 2) return 0;
+    const int fused = (opt && storage != IGR_STORE_F64) ? opt->fused : (storage == IGR_STORE_F64 ? 0 : 1);
+    if (storage < 0 || storage > 3) return 0;
     Grid g = make_grid(nx, ny, nz, storage, nullptr);
-    return make_layout(g, storage, fused, opt ? opt->variant : 0, (opt && opt->n_fluids == 2) ? 7 : 5).total;
+    return make_layout(g, storage, fused, storage == IGR_STORE_F64 ? IGR_VARIANT_SIMPLE : (opt ? opt->variant : 0),
+                       (opt && opt->n_fluids == 2) ? 7 : 5).total;
 }
 
 int igr_create(int nx, int ny, int nz, double dx, double gamma, double alpha, int order,
@@ -295,7 +321,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
         n_jacobi < 0 || (order != 5 && order != 3))
         return IGR_ERR_ARG;
     const int storage = opt ? opt->storage : IGR_STORE_F32;
-    if (storage < 0 || storage > 2) return IGR_ERR_ARG;
+    if (storage < 0 || storage > 3) return IGR_ERR_ARG;
     for (int a = 0; a < 3; ++a) {
         const int lo = bc->face[2 * a], hi = bc->face[2 * a + 1];
         if (lo < 0 || lo > 3 || hi < 0 || hi > 3) return IGR_ERR_BC;
@@ -318,6 +344,10 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     s->storage = storage;
     s->fused = opt ? (opt->fused != 0) : 1;                 // igr_create: the fused (headline) path
     s->variant = opt ? opt->variant : 0;
+    if (storage == IGR_STORE_F64) {                         // fp64 mode: one kernel per row, r materialised
+        if (two) { delete s; return IGR_ERR_ARG; }
+        s->fused = 0; s->variant = IGR_VARIANT_SIMPLE;
+    }
     s->maps.valid = false;
     s->jmaps.valid = false;
     s->order = order; s->n_jacobi = n_jacobi;
@@ -397,13 +427,13 @@ int igr_sync(igr_solver *s)
     return finish(s, "igr_sync");
 }
 
-int igr_set_state(igr_solver *s, const float *q)
+static int set_state_any(igr_solver *s, const void *q, int ubytes)
 {
     if (!s || !q) return IGR_ERR_ARG;
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
     s->cur = 0;
     for (int c = 0; c < s->nf; ++c) {
-        int rc = field_in(s, q + c * n, s->st[0].f[c], s->storage);
+        int rc = field_in(s, (const char *)q + c * n * ubytes, s->st[0].f[c], s->storage, 0, -1, ubytes);
         if (rc != IGR_OK) return rc;
     }
     const size_t qb = (size_t)s->g.np * elem_size(s->storage);
@@ -412,6 +442,28 @@ int igr_set_state(igr_solver *s, const float *q)
     s->sig_cur = 0;
     s->wave_valid = false;
     return finish(s, "igr_set_state");
+}
+
+int igr_set_state(igr_solver *s, const float *q) { return set_state_any(s, q, 4); }
+int igr_set_state_f64(igr_solver *s, const double *q) { return set_state_any(s, q, 8); }
+
+int igr_get_state_f64(igr_solver *s, double *q)
+{
+    if (!s || !q) return IGR_ERR_ARG;
+    const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
+    for (int c = 0; c < s->nf; ++c) {
+        int rc = field_out(s, s->st[s->cur].f[c], q + c * n, s->storage, 0, -1, 8);
+        if (rc != IGR_OK) return rc;
+    }
+    return igr_sync(s);
+}
+
+int igr_get_sigma_f64(igr_solver *s, double *f)
+{
+    if (!s || !f) return IGR_ERR_ARG;
+    int rc = field_out(s, s->sig[s->sig_cur], f, s->storage, 0, -1, 8);
+    if (rc != IGR_OK) return rc;
+    return igr_sync(s);
 }
 
 int igr_set_state_planes(igr_solver *s, int k0, int nk, const float *q)
@@ -454,7 +506,8 @@ int igr_set_sigma(igr_solver *s, const float *f)
     if (!s || !f) return IGR_ERR_ARG;
     int rc = field_in(s, f, s->sig[s->sig_cur], s->storage);
     if (rc != IGR_OK) return rc;
-    launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);
+    if (s->storage == IGR_STORE_F64) launch64_halo_sigma(s->g, (double *)s->sig[s->sig_cur], s->stream);
+    else launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);
     return finish(s, "igr_set_sigma");
 }
 
@@ -469,6 +522,7 @@ int igr_get_sigma(igr_solver *s, float *f)
 int igr_get_source(igr_solver *s, float *f)
 {
     if (!s || !f) return IGR_ERR_ARG;
+    if (s->storage == IGR_STORE_F64) return s->fail(IGR_ERR_ARG, "igr_get_source: not available in the fp64 mode");
     int rc = field_out(s, s->b, f, IGR_STORE_F32);
     if (rc != IGR_OK) return rc;
     return igr_sync(s);
@@ -477,6 +531,7 @@ int igr_get_source(igr_solver *s, float *f)
 int igr_set_source(igr_solver *s, const float *f)
 {
     if (!s || !f) return IGR_ERR_ARG;
+    if (s->storage == IGR_STORE_F64) return s->fail(IGR_ERR_ARG, "igr_set_source: not available in the fp64 mode");
     int rc = field_in(s, f, s->b, IGR_STORE_F32);
     if (rc != IGR_OK) return rc;
     return finish(s, "igr_set_source");
@@ -486,6 +541,7 @@ int igr_get_rhs(igr_solver *s, float *r)
 {
     if (!s || !r) return IGR_ERR_ARG;
     if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: r is never materialised (fused step only)");
+    if (s->storage == IGR_STORE_F64) return s->fail(IGR_ERR_ARG, "igr_get_rhs: not available in the fp64 mode");
     { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     const size_t n = (size_t)s->g.nx * s->g.ny * s->g.nz;
     for (int c = 0; c < 5; ++c) {
@@ -498,6 +554,7 @@ int igr_get_rhs(igr_solver *s, float *r)
 int igr_get_padded(igr_solver *s, int c, float *f)
 {
     if (!s || !f || c < 0 || c > s->nf) return IGR_ERR_ARG;
+    if (s->storage == IGR_STORE_F64) return s->fail(IGR_ERR_ARG, "igr_get_padded: not available in the fp64 mode");
     const Grid &g = s->g;
     const void *field = c < s->nf ? s->st[s->cur].f[c] : s->sig[s->sig_cur];
     const size_t wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG, wz = g.nz + 2 * IGR_NG;
@@ -523,7 +580,8 @@ int igr_halo_bc(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     RowTimer t(s, 0, 1);
-    launch_halo_q(s->g, s->storage, s->st[s->cur], s->bc, s->nf, s->stream);
+    if (s->storage == IGR_STORE_F64) launch64_halo_q(s->g, s->st[s->cur], s->bc64, s->stream);
+    else launch_halo_q(s->g, s->storage, s->st[s->cur], s->bc, s->nf, s->stream);
     return finish(s, "igr_halo_bc");
 }
 
@@ -531,6 +589,10 @@ int igr_sigma_source(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     RowTimer t(s, 1, s->nf == 7 ? 2 : 1);
+    if (s->storage == IGR_STORE_F64) {
+        launch64_source(s->g, s->st[s->cur], (double *)s->b, s->alpha, 1.0 / (2.0 * s->dx), s->stream);
+        return finish(s, "igr_sigma_source");
+    }
     const bool viscous = s->mu > 0 || s->zeta > 0;
     StagePtrs q = s->st[s->cur];
     if (s->nf == 7) {
@@ -548,6 +610,17 @@ int igr_jacobi(igr_solver *s)
 {
     if (!s) return IGR_ERR_ARG;
     const float k2 = (float)(s->alpha / (s->dx * s->dx));
+    if (s->storage == IGR_STORE_F64) {
+        RowTimer t(s, 2, s->n_jacobi + 1);
+        for (int it = 0; it < s->n_jacobi; ++it) {
+            launch64_jacobi_sweep(s->g, (const double *)s->st[s->cur].f[0], (const double *)s->b,
+                                  (const double *)s->sig[s->sig_cur], (double *)s->sig[1 - s->sig_cur],
+                                  s->alpha / (s->dx * s->dx), s->stream);
+            s->sig_cur = 1 - s->sig_cur;
+        }
+        launch64_halo_sigma(s->g, (double *)s->sig[s->sig_cur], s->stream);
+        return finish(s, "igr_jacobi");
+    }
     if (s->variant == IGR_VARIANT_TILED) {
         // temporally blocked: passes of up to 5 sweeps, each ONE read of rho, b, Sigma and one write
         static int maxns = -1;                   // IGR_JACOBI_MAXNS=1..5: sweeps per blocked pass (tuning)
@@ -593,6 +666,12 @@ int igr_rhs(igr_solver *s)
     if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: only the fused step (igr_step / igr_stage) is built");
     { const int rc = ensure_r(s); if (rc != IGR_OK) return rc; }
     RowTimer t(s, 3, 1);
+    if (s->storage == IGR_STORE_F64) {
+        double *r64[5];
+        for (int c = 0; c < 5; ++c) r64[c] = (double *)s->r[c];
+        launch64_rhs(s->g, s->order, s->st[s->cur], (const double *)s->sig[s->sig_cur], r64, s->gamma, s->dx, s->stream);
+        return finish(s, "igr_rhs");
+    }
     RhsParams p;
     p.gamma = (float)s->gamma; p.inv_dx = (float)(1.0 / s->dx); p.order = s->order;
     if (s->variant == IGR_VARIANT_TILED) {
@@ -630,6 +709,17 @@ int igr_rk_update(igr_solver *s, int stage, double dt)
     const float beta = stage == 1 ? 1.0f : (stage == 2 ? 0.25f : (float)(2.0 / 3.0));
     StagePtrs &A = s->st[0], &B = s->st[1];
     RowTimer t(s, 4, 1);
+    if (s->storage == IGR_STORE_F64) {
+        double *r64[5];
+        for (int c = 0; c < 5; ++c) r64[c] = (double *)s->r[c];
+        const double b64 = stage == 1 ? 1.0 : (stage == 2 ? 0.25 : 2.0 / 3.0);
+        if (stage == 3) IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult64), s->stream));
+        launch64_rk_update(s->g, A, stage == 1 ? A : B, stage == 3 ? A : B, r64, b64, dt, s->gamma,
+                           stage == 3 ? (WaveResult64 *)s->wave : nullptr, s->stream);
+        s->cur = stage == 3 ? 0 : 1;
+        s->wave_valid = stage == 3;
+        return finish(s, "igr_rk_update");
+    }
     if (stage == 1) {
         launch_rk_update(s->g, s->storage, A, A, B, s->r, beta, (float)dt, (float)s->gamma, nullptr, s->stream);
         s->cur = 1;
@@ -720,6 +810,7 @@ int igr_export_fields(igr_solver *s, igr_export *out)
 {
     if (!s || !out) return IGR_ERR_ARG;
     if (s->nf != 5) return s->fail(IGR_ERR_ARG, "two fluids: the slab exchange is not built");
+    if (s->storage == IGR_STORE_F64) return s->fail(IGR_ERR_ARG, "fp64 mode: the slab exchange is not built");
     memset(out, 0, sizeof *out);
     out->base = (uint64_t)(uintptr_t)s->base;
     for (int b = 0; b < 3; ++b)
@@ -810,6 +901,25 @@ int igr_set_wave_range(igr_solver *s, int k0, int k1)
 int igr_max_wavespeed(igr_solver *s, double *out)
 {
     if (!s || !out) return IGR_ERR_ARG;
+    if (s->storage == IGR_STORE_F64) {
+        if (!s->wave_valid) {
+            RowTimer t(s, 5, 1);
+            IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult64), s->stream));
+            launch64_wavespeed(s->g, s->st[s->cur], s->gamma, (WaveResult64 *)s->wave, s->stream);
+            s->wave_valid = (s->cur == 0);
+        }
+        WaveResult64 h;
+        IGR_CUDA_OK(cudaMemcpyAsync(&h, s->wave, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+        IGR_CUDA_OK(cudaStreamSynchronize(s->stream));
+        int rc = finish(s, "igr_max_wavespeed");
+        if (rc != IGR_OK) return rc;
+        double v;
+        memcpy(&v, &h.max_bits, 8);
+        *out = v;
+        if (h.nonfinite || !(v > 0.0) || !std::isfinite(v))
+            return s->fail(IGR_ERR_NONFINITE, "igr_max_wavespeed: non-finite state (NaN/Inf, or negative pressure/density)");
+        return IGR_OK;
+    }
     if (!s->wave_valid) {
         RowTimer t(s, 5, 1);
         IGR_CUDA_OK(cudaMemsetAsync(s->wave, 0, sizeof(WaveResult), s->stream));
@@ -837,6 +947,7 @@ int igr_set_viscosity(igr_solver *s, double mu, double zeta)
 {
     if (!s || !(mu >= 0) || !(zeta >= 0)) return IGR_ERR_ARG;
     if (s->nf != 5 && (mu > 0 || zeta > 0)) return s->fail(IGR_ERR_ARG, "two fluids: viscous fluxes are not built");
+    if (s->storage == IGR_STORE_F64 && (mu > 0 || zeta > 0)) return s->fail(IGR_ERR_ARG, "fp64 mode: viscous fluxes are not built");
     if ((mu > 0 || zeta > 0) && !s->tau) {
         if (cudaMalloc((void **)&s->tau, (size_t)s->g.np * 6 * 4) != cudaSuccess) {
             cudaGetLastError();

@@ -69,6 +69,17 @@ struct BcDesc {
     InflowFace inflow[6];
 };
 
+// fp64 mode (IGR_STORE_F64): inflow tables in double, wave result in 64 bits
+struct Inflow64 {
+    const double *weight[6];  // [n1][n0] blend weight per transverse cell (NULL: none)
+    const double *fixed[6];   // [n1][n0][5]
+    int n0[6], n1[6];
+};
+struct WaveResult64 {
+    unsigned long long max_bits;   // double bits of the maximum wave speed (non-negative)
+    unsigned int nonfinite;
+};
+
 // ordered-int encoding of non-negative floats for atomicMax
 struct WaveResult {
     unsigned int max_bits;    // float bits of the maximum wave speed (non-negative)

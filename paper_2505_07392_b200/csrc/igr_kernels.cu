@@ -704,3 +704,364 @@ void launch_viscous_add(const Grid &g, int storage, int order, StagePtrs q, cons
         else k_viscous_add<T, 3><<<grid, 128, 0, st>>>(g, q, tau, r[1], r[2], r[3], r[4], inv_dx);
     });
 }
+
+// =============================================================================== fp64 mode (NEXT-4)
+// IGR_STORE_F64: fp64 storage AND fp64 arithmetic, for a like-for-like column beside the paper's FP64 grind
+// times (Table 1).  One thread per cell, one launch per row and per Jacobi sweep, IEEE
+// division and square root, every formula in the oracle's order (parity <= 1e-12 after several steps).  It is the
+// straightforward form of the hot path: the tiled TMA kernels are fp32 (the precision the paper's large runs and
+// the headline use, L297); B200's plain FP64 rate is half its FP32 rate and the state is twice as large.
+namespace f64 {
+
+__global__ void k_unpack(Grid g, const double *__restrict__ user, double *__restrict__ field, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        field[g.idx(i, (int)(r % g.ny), k0 + (int)(r / g.ny))] = user[t];
+    }
+}
+__global__ void k_unpack32(Grid g, const float *__restrict__ user, double *__restrict__ field, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        field[g.idx(i, (int)(r % g.ny), k0 + (int)(r / g.ny))] = (double)user[t];
+    }
+}
+__global__ void k_pack(Grid g, const double *__restrict__ field, double *__restrict__ user, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        user[t] = field[g.idx(i, (int)(r % g.ny), k0 + (int)(r / g.ny))];
+    }
+}
+__global__ void k_pack32(Grid g, const double *__restrict__ field, float *__restrict__ user, int k0, int nk)
+{
+    long long n = (long long)nk * g.ny * g.nx;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        user[t] = (float)field[g.idx(i, (int)(r % g.ny), k0 + (int)(r / g.ny))];
+    }
+}
+
+// a1: ghosts of q by the index map, blended towards the fixed patch state on inflow faces (reading A8 / A8b)
+__global__ void k_halo_q(Grid g, StagePtrs q, Inflow64 bc)
+{
+    const long long n = ghost_count(g);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        GhostCell c = decode_ghost(g, t);
+        if (ghost_is_external(g, c.i, c.j, c.k)) continue;
+        const long long dst = g.idx(c.i, c.j, c.k);
+        const long long src = g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
+                                    map_index(c.k, g.nz, g.bc[4]));
+        double w = 0.0;
+        const double *fixed = nullptr;
+        const int idx[3] = { c.i, c.j, c.k }, nn[3] = { g.nx, g.ny, g.nz };
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            int face = idx[a] < 0 ? 2 * a : (idx[a] >= nn[a] ? 2 * a + 1 : -1);
+            if (face < 0 || fixed != nullptr || bc.weight[face] == nullptr) continue;
+            int t0 = (a == 0) ? idx[1] : idx[0];
+            int t1 = (a == 2) ? idx[1] : idx[2];
+            if (t0 < 0 || t0 >= bc.n0[face] || t1 < 0 || t1 >= bc.n1[face]) continue;
+            double ww = bc.weight[face][(long long)t1 * bc.n0[face] + t0];
+            if (ww > 0.0) { w = ww; fixed = bc.fixed[face] + ((long long)t1 * bc.n0[face] + t0) * 5; }
+        }
+#pragma unroll
+        for (int cmp = 0; cmp < 5; ++cmp) {
+            double *fld = (double *)q.f[cmp];
+            double v = fld[src];
+            if (fixed != nullptr) v = (w >= 1.0) ? fixed[cmp] : v + w * (fixed[cmp] - v);
+            fld[dst] = v;
+        }
+    }
+}
+
+__global__ void k_halo_sigma(Grid g, double *__restrict__ sig)
+{
+    const long long n = ghost_count(g);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        GhostCell c = decode_ghost(g, t);
+        if (ghost_is_external(g, c.i, c.j, c.k)) continue;
+        sig[g.idx(c.i, c.j, c.k)] = sig[g.idx(map_index(c.i, g.nx, g.bc[0]), map_index(c.j, g.ny, g.bc[2]),
+                                              map_index(c.k, g.nz, g.bc[4]))];
+    }
+}
+
+// a2: b = alpha (tr((grad u)^2) + (tr grad u)^2), central differences of u = m / rho (eq. 9; L132)
+__global__ void k_source(Grid g, StagePtrs q, double *__restrict__ b, double alpha, double inv2dx)
+{
+    const long long st[3] = { 1, g.sy, g.sz };
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    const double *rho = (const double *)q.f[0];
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        const long long id = g.idx(i, (int)(r % g.ny), (int)(r / g.ny));
+        double G[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double *m = (const double *)q.f[1 + a];
+#pragma unroll
+            for (int d = 0; d < 3; ++d)
+                G[a][d] = (m[id + st[d]] / rho[id + st[d]] - m[id - st[d]] / rho[id - st[d]]) * inv2dx;
+        }
+        double trsq = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) trsq += G[a][d] * G[d][a];
+        }
+        const double tr = G[0][0] + G[1][1] + G[2][2];
+        b[id] = alpha * (trsq + tr * tr);
+    }
+}
+
+// a3: one Jacobi sweep; Sigma neighbours through the BC index map, densities from the filled ghosts
+__global__ void k_jacobi_sweep(Grid g, const double *__restrict__ rho, const double *__restrict__ b,
+                               const double *__restrict__ sin, double *__restrict__ sout, double k2)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const long long id = g.idx(i, j, k);
+        const double rc = rho[id];
+        double num = 0.0, den = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int sgn = -1; sgn <= 1; sgn += 2) {
+                int ii = i + (a == 0 ? sgn : 0), jj = j + (a == 1 ? sgn : 0), kk = k + (a == 2 ? sgn : 0);
+                const double w = 2.0 / (rc + rho[g.idx(ii, jj, kk)]);
+                num += w * sin[g.idx(map_index(ii, g.nx, g.bc[0]), map_index(jj, g.ny, g.bc[2]),
+                                     map_index(kk, g.nz, g.bc[4]))];
+                den += w;
+            }
+        }
+        sout[id] = (b[id] + k2 * num) / (1.0 / rc + k2 * den);
+    }
+}
+
+// a4: r = -div F^ (reconstruction L132/L164, primitives from reconstructed values L187-L198, p + Sigma eqs. 6-8,
+// local Lax-Friedrichs L207-L210 with the cell-centred speed of the two adjacent cells, reading A5)
+template <int ORDER>
+__device__ __forceinline__ void reconstruct(const double f[6], double &fl, double &fr)
+{
+    if (ORDER == 5) {
+        fl = (2.0 * f[0] - 13.0 * f[1] + 47.0 * f[2] + 27.0 * f[3] - 3.0 * f[4]) / 60.0;
+        fr = (-3.0 * f[1] + 27.0 * f[2] + 47.0 * f[3] - 13.0 * f[4] + 2.0 * f[5]) / 60.0;
+    } else {
+        fl = (-f[1] + 5.0 * f[2] + 2.0 * f[3]) / 6.0;
+        fr = (2.0 * f[2] + 5.0 * f[3] - f[4]) / 6.0;
+    }
+}
+
+__device__ __forceinline__ void side_flux(int d, double gm1, const double U[5], double sg, double F[5])
+{
+    const double ud = U[1 + d] / U[0];
+    const double p = gm1 * (U[4] - 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / U[0]);
+    F[0] = U[1 + d];
+    F[1] = U[1] * ud; F[2] = U[2] * ud; F[3] = U[3] * ud;
+    F[1 + d] += p + sg;
+    F[4] = (U[4] + p + sg) * ud;
+}
+
+__device__ __forceinline__ double cell_wavespeed(int d, double gamma, const StagePtrs &q, long long id)
+{
+    const double rho = ((const double *)q.f[0])[id];
+    const double mx = ((const double *)q.f[1])[id], my = ((const double *)q.f[2])[id], mz = ((const double *)q.f[3])[id];
+    const double p = (gamma - 1.0) * (((const double *)q.f[4])[id] - 0.5 * (mx * mx + my * my + mz * mz) / rho);
+    const double md = d == 0 ? mx : (d == 1 ? my : mz);
+    return fabs(md / rho) + sqrt(gamma * p / rho);
+}
+
+template <int ORDER>
+__device__ __forceinline__ void face_flux(int d, const StagePtrs &q, const double *sig, long long id, long long stride,
+                                          double gamma, double F[5])
+{
+    double UL[5], UR[5], f[6], sl, sr;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+#pragma unroll
+        for (int t = 0; t < 6; ++t) f[t] = ((const double *)q.f[c])[id + (t - 2) * stride];
+        reconstruct<ORDER>(f, UL[c], UR[c]);
+    }
+#pragma unroll
+    for (int t = 0; t < 6; ++t) f[t] = sig[id + (t - 2) * stride];
+    reconstruct<ORDER>(f, sl, sr);
+    const double lam = fmax(cell_wavespeed(d, gamma, q, id), cell_wavespeed(d, gamma, q, id + stride));
+    double FL[5], FR[5];
+    side_flux(d, gamma - 1.0, UL, sl, FL);
+    side_flux(d, gamma - 1.0, UR, sr, FR);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) F[c] = 0.5 * (FL[c] + FR[c]) - 0.5 * lam * (UR[c] - UL[c]);
+}
+
+struct RPtrs { double *r[5]; };
+
+template <int ORDER>
+__global__ void __launch_bounds__(128) k_rhs(Grid g, StagePtrs q, const double *__restrict__ sig, RPtrs rr, double gamma,
+                                             double dx)
+{
+    const long long st[3] = { 1, g.sy, g.sz };
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        const long long id = g.idx(i, (int)(r % g.ny), (int)(r / g.ny));
+        double acc[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            // both faces through ONE instance of the flux code: the two cells of a face see bitwise the same flux
+            double Fp[5], Fm[5];
+#pragma unroll 1
+            for (int side = 0; side < 2; ++side) {
+                double F[5];
+                face_flux<ORDER>(d, q, sig, side ? id - st[d] : id, st[d], gamma, F);
+#pragma unroll
+                for (int c = 0; c < 5; ++c) { if (side) Fm[c] = F[c]; else Fp[c] = F[c]; }
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c) acc[c] -= (Fp[c] - Fm[c]) / dx;
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) rr.r[c][id] = acc[c];
+    }
+}
+
+// a6: max_d |u_d| + c; non-negative doubles order like their bit patterns, so one 64-bit atomicMax per block
+__device__ __forceinline__ void block_reduce_wave(double v, bool bad, WaveResult64 *wave)
+{
+    __shared__ double s_max[32];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) s_bad = 0;
+    __syncthreads();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    bad = __any_sync(0xffffffffu, bad);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { s_max[wid] = v; if (bad) atomicOr(&s_bad, 1); }
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        v = lane < nw ? s_max[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if (lane == 0) {
+            atomicMax(&wave->max_bits, (unsigned long long)__double_as_longlong(v));
+            if (s_bad) atomicOr(&wave->nonfinite, 1u);
+        }
+    }
+}
+
+__device__ __forceinline__ double wavespeed_of(const double o[5], double gamma, bool &bad)
+{
+    const double rho = o[0];
+    const double p = (gamma - 1.0) * (o[4] - 0.5 * (o[1] * o[1] + o[2] * o[2] + o[3] * o[3]) / rho);
+    const double um = fmax(fabs(o[1] / rho), fmax(fabs(o[2] / rho), fabs(o[3] / rho)));
+    const double v = um + sqrt(gamma * p / rho);
+    if (!(v <= 1.0e300)) { bad = true; return 0.0; }
+    return v;
+}
+
+// a5 (+ a6): q_out = q_n + beta ((q_s - q_n) + dt r)  (reading A18)
+template <bool WAVE>
+__global__ void k_rk_update(Grid g, StagePtrs qn, StagePtrs qs, StagePtrs qo, RPtrs rr, double beta, double dt,
+                            double gamma, WaveResult64 *wave)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    double vmax = 0.0;
+    bool bad = false;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int k = (int)(r / g.ny);
+        const long long id = g.idx(i, (int)(r % g.ny), k);
+        double o[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            const double a = ((const double *)qn.f[c])[id], s = ((const double *)qs.f[c])[id];
+            o[c] = a + beta * ((s - a) + dt * rr.r[c][id]);
+            ((double *)qo.f[c])[id] = o[c];
+        }
+        if (WAVE && k >= g.wk0 && k < g.wk1) vmax = fmax(vmax, wavespeed_of(o, gamma, bad));
+    }
+    if (WAVE) block_reduce_wave(vmax, bad, wave);
+}
+
+__global__ void k_wavespeed(Grid g, StagePtrs q, double gamma, WaveResult64 *wave)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    double vmax = 0.0;
+    bool bad = false;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(t % g.nx); long long r = t / g.nx;
+        int k = (int)(r / g.ny);
+        if (k < g.wk0 || k >= g.wk1) continue;
+        const long long id = g.idx(i, (int)(r % g.ny), k);
+        double o[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) o[c] = ((const double *)q.f[c])[id];
+        vmax = fmax(vmax, wavespeed_of(o, gamma, bad));
+    }
+    block_reduce_wave(vmax, bad, wave);
+}
+
+}  // namespace f64
+
+// ---- fp64 launchers (igr_kernels.h)
+void launch64_unpack(const Grid &g, const void *user, int user_is_f32, double *field, int k0, int nk, cudaStream_t st)
+{
+    const long long n = (long long)nk * g.ny * g.nx;
+    if (user_is_f32) f64::k_unpack32<<<blocks_for(n, 256), 256, 0, st>>>(g, (const float *)user, field, k0, nk);
+    else f64::k_unpack<<<blocks_for(n, 256), 256, 0, st>>>(g, (const double *)user, field, k0, nk);
+}
+void launch64_pack(const Grid &g, const double *field, void *user, int user_is_f32, int k0, int nk, cudaStream_t st)
+{
+    const long long n = (long long)nk * g.ny * g.nx;
+    if (user_is_f32) f64::k_pack32<<<blocks_for(n, 256), 256, 0, st>>>(g, field, (float *)user, k0, nk);
+    else f64::k_pack<<<blocks_for(n, 256), 256, 0, st>>>(g, field, (double *)user, k0, nk);
+}
+void launch64_halo_q(const Grid &g, StagePtrs q, const Inflow64 &bc, cudaStream_t st)
+{
+    f64::k_halo_q<<<blocks_for(ghost_count(g), 256, 148 * 16), 256, 0, st>>>(g, q, bc);
+}
+void launch64_halo_sigma(const Grid &g, double *sig, cudaStream_t st)
+{
+    f64::k_halo_sigma<<<blocks_for(ghost_count(g), 256, 148 * 16), 256, 0, st>>>(g, sig);
+}
+void launch64_source(const Grid &g, StagePtrs q, double *b, double alpha, double inv2dx, cudaStream_t st)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    f64::k_source<<<blocks_for(n, 256), 256, 0, st>>>(g, q, b, alpha, inv2dx);
+}
+void launch64_jacobi_sweep(const Grid &g, const double *rho, const double *b, const double *sin, double *sout, double k2,
+                           cudaStream_t st)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    f64::k_jacobi_sweep<<<blocks_for(n, 256), 256, 0, st>>>(g, rho, b, sin, sout, k2);
+}
+void launch64_rhs(const Grid &g, int order, StagePtrs q, const double *sig, double *const r[5], double gamma, double dx,
+                  cudaStream_t st)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    f64::RPtrs rr;
+    for (int c = 0; c < 5; ++c) rr.r[c] = r[c];
+    if (order == 5) f64::k_rhs<5><<<blocks_for(n, 128), 128, 0, st>>>(g, q, sig, rr, gamma, dx);
+    else f64::k_rhs<3><<<blocks_for(n, 128), 128, 0, st>>>(g, q, sig, rr, gamma, dx);
+}
+void launch64_rk_update(const Grid &g, StagePtrs qn, StagePtrs qs, StagePtrs qout, double *const r[5], double beta,
+                        double dt, double gamma, WaveResult64 *wave, cudaStream_t st)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    f64::RPtrs rr;
+    for (int c = 0; c < 5; ++c) rr.r[c] = r[c];
+    const unsigned nb = blocks_for(n, 256, 148 * 8);
+    if (wave) f64::k_rk_update<true><<<nb, 256, 0, st>>>(g, qn, qs, qout, rr, beta, dt, gamma, wave);
+    else f64::k_rk_update<false><<<nb, 256, 0, st>>>(g, qn, qs, qout, rr, beta, dt, gamma, wave);
+}
+void launch64_wavespeed(const Grid &g, StagePtrs q, double gamma, WaveResult64 *wave, cudaStream_t st)
+{
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    f64::k_wavespeed<<<blocks_for(n, 256, 148 * 8), 256, 0, st>>>(g, q, gamma, wave);
+}

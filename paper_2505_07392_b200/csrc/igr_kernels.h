@@ -81,3 +81,18 @@ void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, 
                            const void *sig_in, void *sig_out, float k2, const CUtensorMap *rmap,
                            const CUtensorMap *bmap, const CUtensorMap *smap, const JacobiQuadPlan *skip,
                            cudaStream_t st);
+
+// ---- fp64 mode (IGR_STORE_F64, NEXT-4): fp64 storage and arithmetic, one thread per cell, one launch per row and
+// per sweep (igr_kernels.cu, namespace f64).  `user` arrays are fp64 or fp32 (user_is_f32).
+void launch64_unpack(const Grid &g, const void *user, int user_is_f32, double *field, int k0, int nk, cudaStream_t st);
+void launch64_pack(const Grid &g, const double *field, void *user, int user_is_f32, int k0, int nk, cudaStream_t st);
+void launch64_halo_q(const Grid &g, StagePtrs q, const Inflow64 &bc, cudaStream_t st);
+void launch64_halo_sigma(const Grid &g, double *sig, cudaStream_t st);
+void launch64_source(const Grid &g, StagePtrs q, double *b, double alpha, double inv2dx, cudaStream_t st);
+void launch64_jacobi_sweep(const Grid &g, const double *rho, const double *b, const double *sin, double *sout, double k2,
+                           cudaStream_t st);
+void launch64_rhs(const Grid &g, int order, StagePtrs q, const double *sig, double *const r[5], double gamma, double dx,
+                  cudaStream_t st);
+void launch64_rk_update(const Grid &g, StagePtrs qn, StagePtrs qs, StagePtrs qout, double *const r[5], double beta,
+                        double dt, double gamma, WaveResult64 *wave, cudaStream_t st);
+void launch64_wavespeed(const Grid &g, StagePtrs q, double gamma, WaveResult64 *wave, cudaStream_t st);

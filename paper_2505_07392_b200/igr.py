@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libigr.so")
 
 OK, ERR_ARG, ERR_BC, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
 BC_PERIODIC, BC_EXTRAP, BC_INFLOW, BC_EXTERNAL = 0, 1, 2, 3
-STORE_F32, STORE_F16, STORE_BF16 = 0, 1, 2
+STORE_F32, STORE_F16, STORE_BF16, STORE_F64 = 0, 1, 2, 3
 VARIANT_TILED, VARIANT_SIMPLE = 0, 1
 _STATUS = {0: "IGR_OK", -1: "IGR_ERR_ARG", -2: "IGR_ERR_BC", -3: "IGR_ERR_ALLOC", -4: "IGR_ERR_CUDA",
            -5: "IGR_ERR_NONFINITE"}
@@ -82,6 +82,8 @@ def lib():
                   "igr_set_source", "igr_get_rhs"):
             getattr(L, n).argtypes = [vp, fp]
         L.igr_get_padded.argtypes = [vp, C.c_int, fp]
+        for n in ("igr_set_state_f64", "igr_get_state_f64", "igr_get_sigma_f64"):
+            getattr(L, n).argtypes = [vp, vp]
         L.igr_set_state_planes.argtypes = [vp, C.c_int, C.c_int, fp]
         L.igr_get_state_planes.argtypes = [vp, C.c_int, C.c_int, fp]
         L.igr_max_wavespeed.argtypes = [vp, C.POINTER(C.c_double)]
@@ -121,13 +123,13 @@ def make_bc(faces, patches=None):
     return bc, keep
 
 
-def _addr(a, shape, writable=False):
-    """Raw address of a contiguous fp32 torch tensor (cpu or cuda) or numpy array of `shape`."""
+def _addr(a, shape, writable=False, f64=False):
+    """Raw address of a contiguous fp32 (f64: fp64) torch tensor (cpu or cuda) or numpy array of `shape`."""
     if isinstance(a, torch.Tensor):
-        assert a.dtype == torch.float32 and a.is_contiguous() and tuple(a.shape) == tuple(shape), \
-            (a.dtype, a.shape, shape)
+        assert a.dtype == (torch.float64 if f64 else torch.float32) and a.is_contiguous() \
+            and tuple(a.shape) == tuple(shape), (a.dtype, a.shape, shape)
         return a.data_ptr()
-    assert isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous \
+    assert isinstance(a, np.ndarray) and a.dtype == (np.float64 if f64 else np.float32) and a.flags.c_contiguous \
         and a.shape == tuple(shape), (type(a), getattr(a, "shape", None), shape)
     if writable:
         assert a.flags.writeable
@@ -206,7 +208,20 @@ class Solver:
 
     # ---- igr.h calls
     def set_state(self, q):
+        if q.dtype in (np.float64, torch.float64):           # fp64 arrays: the fp64 mode only (igr_set_state_f64)
+            self._check(lib().igr_set_state_f64(self._h, _addr(q, (self.nf,) + self.shape, f64=True)))
+            return
         self._check(lib().igr_set_state(self._h, _addr(q, (self.nf,) + self.shape)))
+
+    def get_state_f64(self, out=None):
+        out = np.empty((self.nf,) + self.shape, np.float64) if out is None else out
+        self._check(lib().igr_get_state_f64(self._h, _addr(out, (self.nf,) + self.shape, True, f64=True)))
+        return out
+
+    def get_sigma_f64(self, out=None):
+        out = np.empty(self.shape, np.float64) if out is None else out
+        self._check(lib().igr_get_sigma_f64(self._h, _addr(out, self.shape, True, f64=True)))
+        return out
 
     def get_state(self, out=None):
         out = np.empty((self.nf,) + self.shape, np.float32) if out is None else out
