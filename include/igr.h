@@ -227,6 +227,19 @@ int igr_set_neighbor(igr_solver *s, int side, const igr_export *peer, const void
 /* enqueue the copies of q (5 fields of the current buffer) and Sigma from every registered neighbour
  * on the solver's stream; drops the cached wave speed if a plane that entered it is overwritten */
 int igr_pull_halo(igr_solver *s);
+/* Stream-ordered ordering of the exchange between processes (no device synchronisation, no GPU idle time while
+ * the hosts talk): every solver owns two INTERPROCESS events, which = 0 "my stage is complete" and which = 1
+ * "my pulls are complete".  igr_event_handle returns the 64-byte CUDA IPC handle of one of them (created on
+ * first use; the bytes can be shipped to another rank), igr_event_open maps a neighbour's event into this
+ * process, igr_event_record records one of mine on my stream, igr_event_wait makes MY stream wait for a
+ * neighbour's event (cudaStreamWaitEvent: it captures the neighbour's most recent record, so the hosts must
+ * have agreed -- a host-only handshake, dist.py -- that the record was enqueued).  A pull then waits only for
+ * the two neighbours' stage, and the next stage's kernels only for the neighbours' pulls. */
+int igr_event_handle(igr_solver *s, int which, unsigned char handle[64]);
+int igr_event_open(const unsigned char handle[64], void **event);
+int igr_event_close(void *event);
+int igr_event_record(igr_solver *s, int which);
+int igr_event_wait(igr_solver *s, void *event);
 /* planes [k0, k1) (0 <= k0 < k1 <= nz) that enter igr_max_wavespeed and the fused stage-3 reduction;
  * default all.  A slab restricts it to its owned planes: the overlap planes are only exact right after a
  * pull, and the max over ranks of the owned maxima is the global maximum. */

@@ -98,6 +98,7 @@ struct igr_solver {
         const char *base = nullptr;  // the neighbour's allocation as addressable from this process
         int dst = 0, src = 0, count = 0;
     } nb[2];
+    cudaEvent_t ipc_ev[2] = { nullptr, nullptr };   // interprocess events: stage complete / pulls complete
     long long launches = 0;          // kernels launched so far (igr_kernel_launches)
     bool profile = false;            // per-row CUDA-event timing (igr_profile)
     std::vector<cudaEvent_t> ev;     // start/stop pairs
@@ -411,6 +412,8 @@ void igr_destroy(igr_solver *s)
 {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
+    for (int i = 0; i < 2; ++i)
+        if (s->ipc_ev[i]) cudaEventDestroy(s->ipc_ev[i]);
     if (s->tau) cudaFree(s->tau);
     if (s->r_owned) cudaFree(s->r_owned);
     for (void *p : s->bc_allocs) cudaFree(p);
@@ -887,6 +890,61 @@ int igr_pull_halo(igr_solver *s)
         const igr_solver::Neighbor &nb = s->nb[side];
         if (nb.active && nb.dst < s->g.wk1 && nb.dst + nb.count > s->g.wk0) s->wave_valid = false;
     }
+    return IGR_OK;
+}
+
+// ---- interprocess events (igr.h): stream-ordered ordering of the exchange
+static int ensure_event(igr_solver *s, int which)
+{
+    if (s->ipc_ev[which]) return IGR_OK;
+    IGR_CUDA_OK(cudaEventCreateWithFlags(&s->ipc_ev[which], cudaEventDisableTiming | cudaEventInterprocess));
+    // an event that was never recorded counts as complete; record it once so that a neighbour that opens the
+    // handle before the first stage waits on something well defined
+    IGR_CUDA_OK(cudaEventRecord(s->ipc_ev[which], s->stream));
+    return IGR_OK;
+}
+
+int igr_event_handle(igr_solver *s, int which, unsigned char handle[64])
+{
+    if (!s || !handle || which < 0 || which > 1) return IGR_ERR_ARG;
+    { const int rc = ensure_event(s, which); if (rc != IGR_OK) return rc; }
+    cudaIpcEventHandle_t h;
+    static_assert(sizeof h == 64, "cudaIpcEventHandle_t is 64 bytes");
+    IGR_CUDA_OK(cudaIpcGetEventHandle(&h, s->ipc_ev[which]));
+    memcpy(handle, &h, sizeof h);
+    return IGR_OK;
+}
+
+int igr_event_open(const unsigned char handle[64], void **event)
+{
+    if (!handle || !event) return IGR_ERR_ARG;
+    cudaIpcEventHandle_t h;
+    memcpy(&h, handle, sizeof h);
+    cudaEvent_t e = nullptr;
+    if (cudaIpcOpenEventHandle(&e, h) != cudaSuccess) { cudaGetLastError(); *event = nullptr; return IGR_ERR_CUDA; }
+    *event = (void *)e;
+    return IGR_OK;
+}
+
+int igr_event_close(void *event)
+{
+    if (!event) return IGR_ERR_ARG;
+    if (cudaEventDestroy((cudaEvent_t)event) != cudaSuccess) { cudaGetLastError(); return IGR_ERR_CUDA; }
+    return IGR_OK;
+}
+
+int igr_event_record(igr_solver *s, int which)
+{
+    if (!s || which < 0 || which > 1) return IGR_ERR_ARG;
+    { const int rc = ensure_event(s, which); if (rc != IGR_OK) return rc; }
+    IGR_CUDA_OK(cudaEventRecord(s->ipc_ev[which], s->stream));
+    return IGR_OK;
+}
+
+int igr_event_wait(igr_solver *s, void *event)
+{
+    if (!s || !event) return IGR_ERR_ARG;
+    IGR_CUDA_OK(cudaStreamWaitEvent(s->stream, (cudaEvent_t)event, 0));
     return IGR_OK;
 }
 

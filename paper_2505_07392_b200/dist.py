@@ -3,9 +3,13 @@ stage (read
 
 The plan (who owns which planes, which planes move) is slab.py; the copies are igr_pull_halo of the C
 library (cudaMemcpyAsync device-to-device from the neighbour's allocation, opened once with CUDA IPC:
-copy engines over NVLink, no SM time, no staging).  torch.distributed carries only the rendezvous: the
-all-gather of the 240-byte igr_export descriptions at start-up, the barriers that order a pull after the
-neighbours' stage, and the max-reduction of the wave speed (one float per step, CFL condition).
+copy engines over NVLink, no SM time, no staging).  The ORDER of a pull after the neighbours' stage, and of the
+next stage after the neighbours' pulls, is stream-ordered: interprocess CUDA events (igr_event_*), waited for
+with cudaStreamWaitEvent on the solver's stream.  No device synchronisation happens inside a step: the hosts only
+exchange a host-side handshake (a barrier of a gloo group: "my record is enqueued") while the GPUs keep
+running, so a rank's pull waits for its two neighbours and nothing else.  torch.distributed carries the
+rendezvous (all-gather of the igr_export descriptions and of the event handles at start-up), those handshakes,
+and the max-reduction of the wave speed (one float per step, CFL condition).
 `exchange="sendrecv"` moves the same planes with torch.distributed point-to-point calls instead (NCCL
 send/recv over NVLink with the nccl backend; host staging with gloo): the path for nodes where CUDA IPC
 is not permitted.
@@ -57,6 +61,8 @@ class SlabSolver:
         if self.nranks > 1:                       # CFL reduction over the owned planes only
             self.solver.set_wave_range(self.slab.own_lo, self.slab.own_hi)
         self._opened = []
+        self._nb_events = []                      # (stage complete, pulls complete) events of the neighbours
+        self._hgroup = None                       # host-only group for the handshakes of the event ordering
         self._recv = S.receives(self.slab, lambda r: self.peer_slabs[r])
         self._send = S.sends(self.slab, lambda r: self.peer_slabs[r])
         if self.exchange_kind == "ipc":
@@ -86,6 +92,13 @@ class SlabSolver:
                 igr.ipc_close(b)
             self._opened = []
             self.exchange_kind = "sendrecv"
+            return
+        # interprocess events: every rank publishes the handles of its two events, opens its neighbours'
+        handles = _gather_bytes(self.solver.event_handle(0) + self.solver.event_handle(1), self.group)
+        for r in sorted({t.peer for t in self._recv}):
+            self._nb_events.append((igr.event_open(handles[r][:64]), igr.event_open(handles[r][64:])))
+        # the handshakes must not enter the CUDA stream: a gloo group beside an nccl one
+        self._hgroup = self.group if dist.get_backend(self.group) == "gloo" else dist.new_group(backend="gloo")
 
     def connect_local(self, solvers):
         """exchange="local": `solvers[r]` is the SlabSolver of rank r in this process."""
@@ -101,6 +114,10 @@ class SlabSolver:
         for b in self._opened:
             igr.ipc_close(b)
         self._opened = []
+        for pair in self._nb_events:
+            for ev in pair:
+                igr.event_close(ev)
+        self._nb_events = []
         self._barrier()                            # an exporter frees its memory only after every importer unmapped it
         self.solver.close()
 
@@ -132,12 +149,21 @@ class SlabSolver:
         if self.exchange_kind == "local":
             self.solver.pull_halo()               # one process, one stream: already ordered
             return
+        if self.exchange_kind == "ipc":
+            # stream-ordered: no device synchronisation, the GPU never waits for the hosts
+            self.solver.event_record(0)                           # my stage is complete (in stream order)
+            dist.barrier(group=self._hgroup)                      # host only: every rank has ENQUEUED that record
+            for done, _ in self._nb_events:
+                self.solver.event_wait(done)                      # my pulls wait for the neighbours' stage
+            self.solver.pull_halo()
+            self.solver.event_record(1)                           # my pulls are complete
+            dist.barrier(group=self._hgroup)
+            for _, pulled in self._nb_events:
+                self.solver.event_wait(pulled)                    # my next stage waits for the neighbours' pulls
+            return
         self.solver.sync()
         self._barrier()                           # the neighbours' stage is complete
-        if self.exchange_kind == "ipc":
-            self.solver.pull_halo()
-        else:
-            self._sendrecv()
+        self._sendrecv()
         self.solver.sync()
         self._barrier()                           # nobody overwrites planes that are still being read
 

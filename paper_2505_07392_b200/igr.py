@@ -27,7 +27,8 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_rk_update", "igr_get_source", "igr_set_source", "igr_get_rhs", "igr_get_padded",
            "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity", "igr_stage",
            "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo", "igr_set_wave_range", "igr_set_state_planes",
-           "igr_get_state_planes"]
+           "igr_get_state_planes", "igr_set_state_f64", "igr_get_state_f64", "igr_get_sigma_f64",
+           "igr_event_handle", "igr_event_open", "igr_event_close", "igr_event_record", "igr_event_wait"]
 
 
 class IgrError(RuntimeError):
@@ -102,6 +103,11 @@ def lib():
         L.igr_set_neighbor.argtypes = [vp, C.c_int, C.POINTER(Export), vp, C.c_int, C.c_int, C.c_int]
         L.igr_pull_halo.argtypes = [vp]
         L.igr_set_wave_range.argtypes = [vp, C.c_int, C.c_int]
+        L.igr_event_handle.argtypes = [vp, C.c_int, C.POINTER(C.c_ubyte * 64)]
+        L.igr_event_open.argtypes = [C.POINTER(C.c_ubyte * 64), C.POINTER(vp)]
+        L.igr_event_close.argtypes = [vp]
+        L.igr_event_record.argtypes = [vp, C.c_int]
+        L.igr_event_wait.argtypes = [vp, vp]
         L.igr_last_error.argtypes = [vp]
         L.igr_last_error.restype = C.c_char_p
         _lib = L
@@ -143,6 +149,22 @@ def ipc_open(peer):
     if rc != OK:
         raise IgrError(rc, "igr_ipc_open")
     return base.value
+
+
+def event_open(handle_bytes):
+    """This process's handle of another process's interprocess event (64-byte CUDA IPC handle)."""
+    buf = (C.c_ubyte * 64).from_buffer_copy(handle_bytes)
+    ev = C.c_void_p()
+    rc = lib().igr_event_open(C.byref(buf), C.byref(ev))
+    if rc != OK:
+        raise IgrError(rc, "igr_event_open")
+    return ev.value
+
+
+def event_close(ev):
+    rc = lib().igr_event_close(C.c_void_p(ev))
+    if rc != OK:
+        raise IgrError(rc, "igr_event_close")
 
 
 def ipc_close(base):
@@ -266,6 +288,18 @@ class Solver:
         out = np.empty(shp, np.float32) if out is None else out
         self._check(lib().igr_get_padded(self._h, c, _addr(out, shp, True)))
         return out
+
+    # ---- interprocess events (igr.h): which = 0 "stage complete", 1 "pulls complete"
+    def event_handle(self, which):
+        buf = (C.c_ubyte * 64)()
+        self._check(lib().igr_event_handle(self._h, int(which), C.byref(buf)))
+        return bytes(buf)
+
+    def event_record(self, which):
+        self._check(lib().igr_event_record(self._h, int(which)))
+
+    def event_wait(self, ev):
+        self._check(lib().igr_event_wait(self._h, C.c_void_p(ev)))
 
     def max_wavespeed(self):
         v = C.c_double()

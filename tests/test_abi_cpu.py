@@ -21,7 +21,7 @@ def lib():
 def test_library_exports_every_declared_symbol(lib):
     header = open(os.path.join(ROOT, "include", "igr.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = sorted(set(re.findall(r"\b(igr_[a-z_]+)\s*\(", header)))
+    declared = sorted(set(re.findall(r"\b(igr_[a-z0-9_]+)\s*\(", header)))
     assert len(declared) >= 20
     for name in declared:
         assert hasattr(lib, name), name

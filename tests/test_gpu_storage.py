@@ -69,14 +69,19 @@ def test_set_get_roundtrip_is_the_storage_rounding(fmt, mode):
 
 @pytest.mark.parametrize("mode", [dict(fused=1), dict(fused=0)], ids=["tiled_fused", "tiled"])
 @pytest.mark.parametrize("fmt", ["f16", "bf16"])
-@pytest.mark.parametrize("case", ["jets", "tgv"])
+@pytest.mark.parametrize("case", ["jets", "tgv", "tgv_m01"])
 def test_three_steps_vs_emulating_and_pure_oracle(case, fmt, mode):
     f = FMT[fmt]
     if case == "jets":
         w = W.jets33(n=64, radius=6, rings=((10, 3),))
     else:
         w = W.taylor_green(48)
-        w.params["mach"] = 0.5          # p0 ~ 2.9: stays well inside the fp16 range and resolution
+        # "tgv": Mach 0.5, p0 ~ 2.9, well inside the resolution of the 2-byte formats.  "tgv_m01": config 3's own
+        # Mach 0.1 (p0 ~ 71, E ~ 178): one ulp of fp16 at E is 0.125, more than the whole pressure variation of the
+        # vortex -- the stored field barely moves (PAPER.md L351 sees the same effect), but GPU and the
+        # storage-emulating oracle must still round alike
+        if case == "tgv":
+            w.params["mach"] = 0.5
     g, emu, pure = run_three(w, fmt, mode)
     got = g.get_state()
     # (a) storage-emulating oracle: the stored values agree except for rare 1-ulp rounding flips
