@@ -373,6 +373,9 @@ JacobiQuadPlan jacobi_quad_plan(const Grid &g, int ns, float k2)
     if (nch < 1) nch = 1;
     int zc = (int)((g.nz + nch - 1) / nch);
     if (zc < 8 * ns) zc = 8 * ns;
+    static int force_zc = -1;                    // IGR_JACOBI_ZC=n: planes per z chunk (tuning)
+    if (force_zc < 0) { const char *e = getenv("IGR_JACOBI_ZC"); force_zc = e ? atoi(e) : 0; }
+    if (force_zc >= 8 * ns) zc = force_zc;
     if (zc > g.nz) zc = g.nz;
     pl.zc = zc;
     return pl;

@@ -103,28 +103,30 @@ void launch_pack_padded(const Grid &g, int storage, const void *field, float *us
 // All ghosts read interior cells only, so one launch covers the three slabs (no ordering).
 struct GhostCell { int i, j, k; bool valid; };
 
-__device__ __forceinline__ GhostCell decode_ghost(const Grid &g, long long t)
+// (unsigned 32-bit arithmetic: the ghost cells of any grid that fits the device number far below 2^32, and a
+// 64-bit division costs five times a 32-bit one; the halo kernels were spending their time here)
+__device__ __forceinline__ GhostCell decode_ghost(const Grid &g, long long t64)
 {
-    const int wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG;
-    const long long nZ = 2LL * IGR_NG * wy * wx;                 // full padded planes below/above
-    const long long nY = (long long)g.nz * 2 * IGR_NG * wx;      // rows in front/behind, interior k
-    const long long nX = (long long)g.nz * g.ny * 2 * IGR_NG;    // columns left/right, interior j, k
+    const unsigned wx = g.nx + 2 * IGR_NG, wy = g.ny + 2 * IGR_NG;
+    const unsigned nZ = 2u * IGR_NG * wy * wx;                   // full padded planes below/above
+    const unsigned nY = (unsigned)g.nz * 2u * IGR_NG * wx;       // rows in front/behind, interior k
+    const unsigned nX = (unsigned)g.nz * (unsigned)g.ny * 2u * IGR_NG;   // columns left/right, interior j, k
+    unsigned t = (unsigned)t64;
     GhostCell c;
     c.valid = true;
     if (t < nZ) {
-        int i = (int)(t % wx); long long r = t / wx;
-        int j = (int)(r % wy), kk = (int)(r / wy);
-        c.i = i - IGR_NG; c.j = j - IGR_NG; c.k = kk < IGR_NG ? kk - IGR_NG : g.nz + (kk - IGR_NG);
+        const unsigned r = t / wx, i = t - r * wx, kk = r / wy, j = r - kk * wy;
+        c.i = (int)i - IGR_NG; c.j = (int)j - IGR_NG; c.k = kk < IGR_NG ? (int)kk - IGR_NG : g.nz + ((int)kk - IGR_NG);
     } else if (t < nZ + nY) {
         t -= nZ;
-        int i = (int)(t % wx); long long r = t / wx;
-        int jj = (int)(r % (2 * IGR_NG)); c.k = (int)(r / (2 * IGR_NG));
-        c.i = i - IGR_NG; c.j = jj < IGR_NG ? jj - IGR_NG : g.ny + (jj - IGR_NG);
+        const unsigned r = t / wx, i = t - r * wx, k = r / (2u * IGR_NG), jj = r - k * (2u * IGR_NG);
+        c.k = (int)k;
+        c.i = (int)i - IGR_NG; c.j = jj < IGR_NG ? (int)jj - IGR_NG : g.ny + ((int)jj - IGR_NG);
     } else if (t < nZ + nY + nX) {
         t -= nZ + nY;
-        int ii = (int)(t % (2 * IGR_NG)); long long r = t / (2 * IGR_NG);
-        c.j = (int)(r % g.ny); c.k = (int)(r / g.ny);
-        c.i = ii < IGR_NG ? ii - IGR_NG : g.nx + (ii - IGR_NG);
+        const unsigned r = t / (2u * IGR_NG), ii = t - r * (2u * IGR_NG), k = r / (unsigned)g.ny, j = r - k * (unsigned)g.ny;
+        c.j = (int)j; c.k = (int)k;
+        c.i = ii < IGR_NG ? (int)ii - IGR_NG : g.nx + ((int)ii - IGR_NG);
     } else {
         c.valid = false; c.i = c.j = c.k = 0;
     }

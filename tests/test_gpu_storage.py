@@ -90,8 +90,12 @@ def test_three_steps_vs_emulating_and_pure_oracle(case, fmt, mode):
     print("stored q: identical %.4f within-1-ulp %.5f worst %.1f ulp; Sigma: %.4f %.5f %.1f"
           % (same, within1, worst, same_s, within1_s, worst_s))
     # a flipped rounding (fp32 vs fp64 arithmetic before the store) is 1 ulp; it can grow by a few
-    # ulps through the following stages, never more
-    assert same >= 0.97 and within1 >= 0.999 and worst <= 8.0, (same, within1, worst)
+    # ulps through the following stages, never more.  Bounds as in DESIGN.md section 7; measured on the B200
+    # (profiles/r02_storage_fractions.txt): identical 0.975-0.995, within 1 ulp >= 0.9998, worst 4.0 ulp.  At
+    # Mach 0.1 the increments dt r are a fraction of an ulp of fp16, so many stores sit near a rounding tie:
+    # identical 0.909 (f16) / 0.970 (bf16), but every value within 1 ulp (worst 0.5)
+    min_same = 0.90 if case == "tgv_m01" else 0.97
+    assert same >= min_same and within1 >= 0.999 and worst <= 8.0, (same, within1, worst)
     assert within1_s >= 0.99 and worst_s <= 16.0, (same_s, within1_s, worst_s)
     # (b) pure fp64 oracle: looser bounds from 9 stores x half an ulp
     mx, l1 = parity.worst(got, pure.get_state())
