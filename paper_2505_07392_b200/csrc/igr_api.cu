@@ -67,6 +67,7 @@ struct igr_solver {
     Grid g;
     int storage = 0, fused = 0, variant = 0, order = 5, n_jacobi = 5;
     RhsTileMaps maps;
+    SourceMaps smaps[3];             // TMA maps of the source kernel, one set per state buffer
     JacobiMaps jmaps;                // TMA maps of the blocked Jacobi kernel
     double dx = 0, gamma = 0, alpha = 0;
     int nf = 5;                      // conserved fields: 5, or 7 with two fluids (NEXT-3, reading A21)
@@ -351,6 +352,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     }
     s->maps.valid = false;
     s->jmaps.valid = false;
+    for (int b = 0; b < 3; ++b) s->smaps[b].valid = false;
     s->order = order; s->n_jacobi = n_jacobi;
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
     s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
@@ -394,6 +396,11 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
         if (rhs_tile_make_maps(s->g, storage, s->st, L.n_state, s->sig, s->nf, &s->maps, &msg) != 0) {
             igr_destroy(s);
             return IGR_ERR_CUDA;
+        }
+        for (int b = 0; b < 3; ++b) {        // (rho, m) of every state buffer for the source kernel
+            const StagePtrs &sp = s->st[b < L.n_state ? b : L.n_state - 1];
+            void *f4[4] = { two ? (void *)s->rhot : sp.f[0], sp.f[two ? 2 : 1], sp.f[two ? 3 : 2], sp.f[two ? 4 : 3] };
+            if (source_make_maps(s->g, storage, f4, &s->smaps[b]) != 0) { igr_destroy(s); return IGR_ERR_CUDA; }
         }
         // the density the Sigma equation reads: field 0 of the state, or the mixture density (two fluids)
         StagePtrs rho_of[3];
@@ -604,8 +611,13 @@ int igr_sigma_source(igr_solver *s)
         launch_rho_total(s->g, (const float *)q.f[0], (const float *)q.f[1], s->rhot, s->stream);
         q.f[0] = s->rhot; q.f[1] = s->st[s->cur].f[2]; q.f[2] = s->st[s->cur].f[3]; q.f[3] = s->st[s->cur].f[4];
     }
-    launch_source(s->g, s->storage, q, s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
-                  viscous ? s->tau : nullptr, (float)s->mu, (float)s->zeta, s->stream);
+    static int no_tma = -1;                  // IGR_SOURCE_TMA=0: the per-thread-load kernel (tuning)
+    if (no_tma < 0) { const char *e = getenv("IGR_SOURCE_TMA"); no_tma = (e && atoi(e) == 0) ? 1 : 0; }
+    if (s->variant == IGR_VARIANT_TILED && !viscous && !no_tma && s->smaps[s->cur].valid)
+        launch_source_tma(s->g, s->storage, s->smaps[s->cur], s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)), s->stream);
+    else
+        launch_source(s->g, s->storage, q, s->b, (float)s->alpha, (float)(1.0 / (2.0 * s->dx)),
+                      viscous ? s->tau : nullptr, (float)s->mu, (float)s->zeta, s->stream);
     return finish(s, "igr_sigma_source");
 }
 

@@ -36,6 +36,15 @@ void launch_halo_sigma(const Grid &g, int storage, void *sig, cudaStream_t st);
 // also written when not NULL
 void launch_source(const Grid &g, int storage, StagePtrs q, float *b, float alpha, float inv2dx,
                    float *tau, float mu, float zeta, cudaStream_t st);
+// a2, TMA-staged form (igr_source_tma.cu): b only (the stress fields of the viscous variant stay with launch_source).
+// f: the padded fields rho, m_x, m_y, m_z in the storage type (two fluids: rho = the fp32 mixture density).
+struct SourceMaps {
+    CUtensorMap f[4];
+    bool valid;
+};
+int source_make_maps(const Grid &g, int storage, void *const f[4], SourceMaps *out);
+void launch_source_tma(const Grid &g, int storage, const SourceMaps &m, float *b, float alpha, float inv2dx,
+                       cudaStream_t st);
 // ghosts of nf derived fp32 fields (stride g.np) by the BC index map
 void launch_halo_fields(const Grid &g, float *base, int nf, cudaStream_t st);
 // NEXT-1, simple form: r[1..4] += -div F_visc (eqs. 2, 3, 5); tau must have its ghosts filled
