@@ -68,7 +68,8 @@ struct igr_solver {
     int storage = 0, fused = 0, variant = 0, order = 5, n_jacobi = 5;
     RhsTileMaps maps;
     SourceMaps smaps[3];             // TMA maps of the source kernel, one set per state buffer
-    JacobiMaps jmaps;                // TMA maps of the blocked Jacobi kernel
+    JacobiMaps jmaps;                // TMA maps of the blocked Jacobi kernel (32-row boxes)
+    JacobiMaps jmaps2;               // the same with 34-row boxes (quad regions 24 rows apart)
     double dx = 0, gamma = 0, alpha = 0;
     int nf = 5;                      // conserved fields: 5, or 7 with two fluids (NEXT-3, reading A21)
     double gamma2 = 0;               // two fluids: exponent of fluid 2
@@ -352,6 +353,7 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
     }
     s->maps.valid = false;
     s->jmaps.valid = false;
+    s->jmaps2.valid = false;
     for (int b = 0; b < 3; ++b) s->smaps[b].valid = false;
     s->order = order; s->n_jacobi = n_jacobi;
     s->dx = dx; s->gamma = gamma; s->alpha = alpha;
@@ -405,7 +407,8 @@ int igr_create_ex(int nx, int ny, int nz, double dx, double gamma, double alpha,
         // the density the Sigma equation reads: field 0 of the state, or the mixture density (two fluids)
         StagePtrs rho_of[3];
         for (int b = 0; b < 3; ++b) { rho_of[b] = s->st[b]; if (two) rho_of[b].f[0] = s->rhot; }
-        if (jacobi_make_maps(s->g, storage, rho_of, L.n_state, s->sig, s->b, &s->jmaps) != 0) {
+        if (jacobi_make_maps(s->g, storage, rho_of, L.n_state, s->sig, s->b, &s->jmaps) != 0 ||
+            jacobi_make_maps(s->g, storage, rho_of, L.n_state, s->sig, s->b, &s->jmaps2, 34) != 0) {
             igr_destroy(s);
             return IGR_ERR_CUDA;
         }
@@ -657,9 +660,11 @@ int igr_jacobi(igr_solver *s)
                                   s->sig[s->sig_cur], s->sig[1 - s->sig_cur], k2,
                                   tma ? &s->jmaps.rho[s->cur] : nullptr, tma ? &s->jmaps.b : nullptr,
                                   tma ? &s->jmaps.sig[s->sig_cur] : nullptr, &quad, s->stream);
-            if (quad.nbx > 0)
-                launch_jacobi_quad(s->g, s->storage, ns, quad, s->sig[1 - s->sig_cur], k2, &s->jmaps.rho[s->cur],
-                                   &s->jmaps.b, &s->jmaps.sig[s->sig_cur], s->stream);
+            if (quad.nbx > 0) {
+                const JacobiMaps &jm = quad.wy ? s->jmaps2 : s->jmaps;
+                launch_jacobi_quad(s->g, s->storage, ns, quad, s->sig[1 - s->sig_cur], k2, &jm.rho[s->cur], &jm.b,
+                                   &jm.sig[s->sig_cur], s->stream);
+            }
             s->sig_cur = 1 - s->sig_cur;
         }
         launch_halo_sigma(s->g, s->storage, s->sig[s->sig_cur], s->stream);

@@ -57,7 +57,7 @@ k_jacobi_blocked(const __grid_constant__ CUtensorMap rmap, const __grid_constant
 {
     // regions taken by k_jacobi_quad (CTA-uniform)
     if ((int)blockIdx.x >= skip.bx0 && (int)blockIdx.x < skip.bx0 + skip.nbx && (int)blockIdx.y >= skip.by0 &&
-        (int)blockIdx.y < skip.by0 + skip.nby)
+        (int)blockIdx.y < skip.by0 + skip.nby_blocked)
         return;
     constexpr int OT = R - 2 * NS;
     constexpr int NTHREADS = R * R / CPT;
@@ -368,26 +368,26 @@ int jacobi_blocked_zc(const Grid &g, int ns)
 namespace {
 
 // 3-D map (x, y, z) of one padded field; box = region + 16 bytes in x (the box start is rounded down to 16 B)
-bool encode_plane_map(CUtensorMap *out, const Grid &g, const void *base, int storage)
+bool encode_plane_map(CUtensorMap *out, const Grid &g, const void *base, int storage, int rows)
 {
     const size_t es = storage == 0 ? 4 : 2;
     cuuint64_t dims[3] = { (cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz };
     cuuint64_t strides[2] = { (cuuint64_t)g.px * es, (cuuint64_t)g.px * g.py * es };
-    cuuint32_t box[3] = { (cuuint32_t)(R + 16 / es), R, 1 };     // 16 bytes wider than the region
+    cuuint32_t box[3] = { (cuuint32_t)(R + 16 / es), (cuuint32_t)rows, 1 };     // 16 bytes wider than the region
     return igr_tma::encode(out, igr_tma::data_type(storage), 3, base, dims, strides, box);
 }
 
 }  // namespace
 
 int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
-                     const float *b, JacobiMaps *out)
+                     const float *b, JacobiMaps *out, int rows)
 {
     out->valid = false;
     for (int i = 0; i < 3; ++i)
-        if (!encode_plane_map(&out->rho[i], g, st[i < n_state ? i : n_state - 1].f[0], storage)) return 1;
+        if (!encode_plane_map(&out->rho[i], g, st[i < n_state ? i : n_state - 1].f[0], storage, rows)) return 1;
     for (int i = 0; i < 2; ++i)
-        if (!encode_plane_map(&out->sig[i], g, sig[i], storage)) return 1;
-    if (!encode_plane_map(&out->b, g, b, 0)) return 1;
+        if (!encode_plane_map(&out->sig[i], g, sig[i], storage, rows)) return 1;
+    if (!encode_plane_map(&out->b, g, b, 0, rows)) return 1;
     out->valid = true;
     return 0;
 }
@@ -439,7 +439,7 @@ void launch_jacobi_blocked(const Grid &g, int storage, int ns, const void *rho, 
     if (sk.nbx > 0 && sk.nby > 0) {
         // every region is taken by the quad kernel: nothing to launch
         const int ot = R - 2 * ns;
-        if (sk.bx0 == 0 && sk.by0 == 0 && sk.nbx >= (g.nx + ot - 1) / ot && sk.nby >= (g.ny + ot - 1) / ot) return;
+        if (sk.bx0 == 0 && sk.by0 == 0 && sk.nbx >= (g.nx + ot - 1) / ot && sk.nby_blocked >= (g.ny + ot - 1) / ot) return;
     }
     if (storage == 0) launch_ns<float>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, sk, st);
     else if (storage == 1) launch_ns<__half>(g, ns, rho, b, sig_in, sig_out, k2, rmap, bmap, smap, sk, st);

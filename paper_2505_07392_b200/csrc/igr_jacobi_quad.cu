@@ -30,7 +30,6 @@ namespace {
 constexpr int R = 32;                       // region edge = warp width
 constexpr int PF = 3;                       // planes in flight (TMA)
 constexpr int NSLOT = PF + 2;               // + the plane that enters and the one before (its halo rows are still read)
-constexpr int SUB = (R + 4) * R;            // floats of one staged field: a box of (R + 16 bytes) x R
 constexpr int SBW = 12;                     // CTAs are ordered in strips of SBW regions: one wave of 148 is compact
 
 __device__ __forceinline__ float rcp_approx(float x)
@@ -40,14 +39,20 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
-// QR = rows per thread (4: 8 warps x 255 registers; 2: 16 warps x 128 registers)
-template <typename T, int NS, int QR>
+// QR = rows per thread (4: 8 warps x 255 registers; 2: 16 warps x 128 registers).
+// WY: the staged boxes hold the row above and the row below the 32 thread rows as well (34 rows).  Those two rows only
+// ever provide the level-0 iterate and the density, which come from the staged planes anyway, so the dependency cone
+// starts one row further out and 24 rows of a region are output instead of 22, at no cost (used when every y region is
+// taken by this kernel, i.e. y is not periodic: the regions then need not line up with those of k_jacobi_blocked).
+template <typename T, int NS, int QR, bool WY>
 __global__ void __launch_bounds__(R * (R / QR), 1)
 k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ CUtensorMap bmap,
               const __grid_constant__ CUtensorMap smap, Grid g, T *__restrict__ sout, float k2, int zc,
               int bx0, int by0, int nbx, int nby)
 {
-    constexpr int OT = R - 2 * NS;
+    constexpr int OT = R - 2 * NS, OTY = WY ? OT + 2 : OT, HY = WY ? NS - 1 : NS;   // outputs per region, y halo rows
+    constexpr int ROWS = WY ? R + 2 : R, R0 = WY ? 1 : 0;  // staged rows, staged row of thread row 0
+    constexpr int SUB = ((R + 4) * ROWS + 31) / 32 * 32;   // floats of one staged field (128-byte multiple: TMA)
     constexpr int NW = R / QR;                             // warps per CTA
     constexpr int NL = NS > 1 ? NS - 1 : 1;                // levels whose edge rows are exchanged
     extern __shared__ __align__(128) float jq_smem[];
@@ -72,7 +77,7 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
         bx += bx0; by += by0;
     }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, row0 = w * QR;
-    const int gi_lo = bx * OT - NS, gj_lo = by * OT - NS;          // region origin (inside the domain)
+    const int gi_lo = bx * OT - NS, gj_lo = by * OTY - HY;         // first thread column / row of the region
     const int kz0 = bz * zc, nkz = min(zc, g.nz - kz0);
     const bool per_z = g.bc[4] == 0;
     const unsigned usz = (unsigned)g.sz;
@@ -81,9 +86,10 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
     // rounded down to 16 bytes; the columns sit `sh` elements into each row
     constexpr int ALT = 16 / (int)sizeof(T), BWT = R + ALT, BWB = R + 4;
     const int xcol = g.gx + gi_lo, shT = xcol & (ALT - 1), shB = xcol & 3;
-    const int own_t = row0 * BWT + shT + lane, own_b = row0 * BWB + shB + lane;
-    const int up_t = max(row0 - 1, 0) * BWT + shT + lane;          // row above / below the quad (own row at the
-    const int dn_t = min(row0 + QR, R - 1) * BWT + shT + lane;     // region edge: outside the dependency cone)
+    const int own_t = (row0 + R0) * BWT + shT + lane, own_b = (row0 + R0) * BWB + shB + lane;
+    // row above / below the quad (without WY the own row at the region edge: outside the dependency cone)
+    const int up_t = (WY ? row0 : max(row0 - 1, 0)) * BWT + shT + lane;
+    const int dn_t = (WY ? row0 + QR + 1 : min(row0 + QR, R - 1)) * BWT + shT + lane;
     // one elected lane of warp 0: plane p of the three fields -> a staging slot.  Everything it needs is
     // warp-uniform (uniform registers, no broadcast loops): the z index of the plane is a running counter kept
     // by all threads (periodic z: wrapped; otherwise rho keeps the first ghost layer, whose density enters the
@@ -98,10 +104,10 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
         float *st = STG + stage * 3 * SUB;
         const int zr = (per_z ? pwrap : min(max(p, -1), g.nz)) + IGR_NG;
         const int zm = (per_z ? pwrap : min(max(p, 0), g.nz - 1)) + IGR_NG;
-        igr_tma::mbar_expect_tx(&full[stage], R * (2 * BWT * (int)sizeof(T) + BWB * 4));
-        igr_tma::tma_load_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo, zr, &full[stage]);
-        igr_tma::tma_load_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo, zm, &full[stage]);
-        igr_tma::tma_load_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo, zm, &full[stage]);
+        igr_tma::mbar_expect_tx(&full[stage], ROWS * (2 * BWT * (int)sizeof(T) + BWB * 4));
+        igr_tma::tma_load_3d(st, &rmap, xcol - shT, IGR_NG + gj_lo - R0, zr, &full[stage]);
+        igr_tma::tma_load_3d(st + SUB, &bmap, xcol - shB, IGR_NG + gj_lo - R0, zm, &full[stage]);
+        igr_tma::tma_load_3d(st + 2 * SUB, &smap, xcol - shT, IGR_NG + gj_lo - R0, zm, &full[stage]);
     };
 
     // edge rows of the quads, levels 1 .. NS-1, double-buffered by plane parity: [par][l - 1][warp][top | bottom][32].
@@ -117,7 +123,7 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
 #pragma unroll
     for (int r = 0; r < QR; ++r) {
         const int ry = row0 + r;
-        if (lane >= NS && lane < R - NS && ry >= NS && ry < R - NS && gi_lo + lane < g.nx && gj_lo + ry < g.ny)
+        if (lane >= NS && lane < R - NS && ry >= HY && ry < R - HY && gi_lo + lane < g.nx && gj_lo + ry < g.ny)
             cmask |= 1u << r;
     }
     // element (gi, gj of row 0, plane kz0) of the output; rows are g.sy apart, planes g.sz
@@ -325,19 +331,19 @@ k_jacobi_quad(const __grid_constant__ CUtensorMap rmap, const __grid_constant__ 
     }
 }
 
-template <typename T, int NS, int QR>
+template <typename T, int NS, int QR, bool WY>
 void launch_quad(const Grid &g, const JacobiQuadPlan &pl, void *sout, float k2, const CUtensorMap &rm,
                  const CUtensorMap &bm, const CUtensorMap &sm, cudaStream_t st)
 {
-    constexpr int NL = NS > 1 ? NS - 1 : 1, NW = R / QR;
+    constexpr int NL = NS > 1 ? NS - 1 : 1, NW = R / QR, ROWS = WY ? R + 2 : R, SUB = ((R + 4) * ROWS + 31) / 32 * 32;
     constexpr int smem = (NSLOT * 3 * SUB + NL * 2 * NW * 2 * 32) * 4 + NSLOT * 8 + 8;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_jacobi_quad<T, NS, QR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaFuncSetAttribute(k_jacobi_quad<T, NS, QR, WY>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         configured = true;
     }
     const int nch = (g.nz + pl.zc - 1) / pl.zc;
-    k_jacobi_quad<T, NS, QR><<<pl.nbx * pl.nby * nch, R * NW, smem, st>>>(rm, bm, sm, g, (T *)sout, k2, pl.zc, pl.bx0,
+    k_jacobi_quad<T, NS, QR, WY><<<pl.nbx * pl.nby * nch, R * NW, smem, st>>>(rm, bm, sm, g, (T *)sout, k2, pl.zc, pl.bx0,
                                                                       pl.by0, pl.nbx, pl.nby);
 }
 
@@ -367,6 +373,9 @@ JacobiQuadPlan jacobi_quad_plan(const Grid &g, int ns, float k2)
     }
     pl.bx0 = lo[0]; pl.by0 = lo[1];
     pl.nbx = hi[0] - lo[0] + 1; pl.nby = hi[1] - lo[1] + 1;
+    // y not periodic: every y region is taken here, so the regions may be 24 rows apart (34-row boxes, WY)
+    pl.nby_blocked = pl.nby;
+    if (g.bc[2] != 0) { pl.wy = 1; pl.nby = (g.ny + ot + 1) / (ot + 2); }
     // z chunks: one per region unless the grid is too small to fill the machine
     // z chunks: enough CTAs to fill the machine, and chunks of at most 512 planes: CTAs are not synchronised with each
     // other, and the shorter their march the less neighbouring regions drift apart along z, i.e. the more of the
@@ -392,10 +401,11 @@ void launch_jacobi_quad(const Grid &g, int storage, int ns, const JacobiQuadPlan
     if (pl.nbx <= 0 || ns != 5) return;
     static int qr = -1;                          // IGR_JACOBI_QR=2|4: rows per thread (tuning)
     if (qr < 0) { const char *e = getenv("IGR_JACOBI_QR"); qr = (e && atoi(e) == 2) ? 2 : 4; }
-#define IGR_JQ(TT)                                                                         \
-    do {                                                                                   \
-        if (qr == 2) launch_quad<TT, 5, 2>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);   \
-        else launch_quad<TT, 5, 4>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);           \
+#define IGR_JQ(TT)                                                                                   \
+    do {                                                                                             \
+        if (pl.wy) launch_quad<TT, 5, 4, true>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);         \
+        else if (qr == 2) launch_quad<TT, 5, 2, false>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st); \
+        else launch_quad<TT, 5, 4, false>(g, pl, sig_out, k2, *rmap, *bmap, *smap, st);              \
     } while (0)
     if (storage == 0) IGR_JQ(float);
     else if (storage == 1) IGR_JQ(__half);

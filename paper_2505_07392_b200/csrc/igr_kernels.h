@@ -75,13 +75,15 @@ struct JacobiMaps {
     CUtensorMap rho[3], sig[2], b;
     bool valid;
 };
+// rows: box height (32: the blocked kernel and quad regions 22 rows apart; 34: quad regions 24 rows apart)
 int jacobi_make_maps(const Grid &g, int storage, const StagePtrs st[3], int n_state, void *const sig[2],
-                     const float *b, JacobiMaps *out);
+                     const float *b, JacobiMaps *out, int rows = 32);
 // a3 (quad form, igr_jacobi_quad.cu): the same blocked pass for the regions (bx, by), bx0 <= bx < bx0 + nbx,
 // by0 <= by < by0 + nby, that need no periodic wrap in x / y; four y-adjacent columns per thread.  nbx = 0: none.
 struct JacobiQuadPlan {
     int bx0, by0, nbx, nby, zc;
-};
+    int wy, nby_blocked;   // wy: regions 24 rows apart with 34-row boxes (TMA maps of jacobi_make_maps(..., rows = 34));
+};                         // nby_blocked: the same y range counted in regions of the blocked kernel's grid (skip test)
 JacobiQuadPlan jacobi_quad_plan(const Grid &g, int ns, float k2);
 void launch_jacobi_quad(const Grid &g, int storage, int ns, const JacobiQuadPlan &pl, void *sig_out, float k2,
                         const CUtensorMap *rmap, const CUtensorMap *bmap, const CUtensorMap *smap, cudaStream_t st);
