@@ -81,32 +81,61 @@ template <> __device__ __forceinline__ float lds<__half>(const __half *p) { retu
 template <> __device__ __forceinline__ float lds<__nv_bfloat16>(const __nv_bfloat16 *p) { return __bfloat162float(*p); }
 
 // ---- numerical flux at one face from the six stencil cells of the six fields.
-// t[f][s]: field f (rho, mx, my, mz, E, Sigma), stencil cell s = 0..5 <-> cells -2..3 about the face.
+// t[p][s]: field pair p (struct Pairs), stencil cell s = 0..5 <-> cells -2..3 about the face.
 // Returns G = 2 F^ = (F_L + F_R) - lambda (U_R - U_L); the factor 1/2 is folded into the divergence.
 // Written with explicit round-to-nearest intrinsics (never contracted or re-associated), so that every
 // inlined instance -- main path, edge warps, neighbouring CTAs -- produces bitwise the same flux from
 // the same inputs (conservation to round-off; uniform states preserved exactly, P7/P8).
+// Packed arithmetic (sm_100: FFMA2 / FADD2 / FMUL2, two fp32 operations per issue slot, each rounded exactly like the
+// scalar instruction).  The fields and the flux components travel in PAIRS: one packed instruction serves two fields.
+// The kernel is bound by instruction issue, so this is where the time goes; the pairs are chosen so that no
+// value ever has to be moved between register pairs.
+typedef float2 f2;
+__device__ __forceinline__ f2 splat(float c) { return make_float2(c, c); }
+__device__ __forceinline__ f2 fsub2(f2 a, f2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }   // FADD2 a, -b
+
+// NF = 5: (m_x, m_y), (m_z, E), (rho, Sigma);  NF = 7: (a1 rho1, a2 rho2), (m_x, m_y), (m_z, E), (a1, Sigma).
+// Flux components sit where their field sits; the face velocity u^ of two fluids takes Sigma's place.
+template <int NF>
+struct Pairs {
+    static constexpr int NP = (NF + 1) / 2;
+    __host__ __device__ static constexpr int fa(int p) { return NF == 5 ? (p == 2 ? 0 : 2 * p + 1) : 2 * p; }
+    __host__ __device__ static constexpr int fb(int p) { return NF == 5 ? (p == 2 ? 5 : 2 * p + 2) : 2 * p + 1; }
+    __host__ __device__ static constexpr int pr(int f) { return NF == 5 ? ((f == 0 || f == 5) ? 2 : (f - 1) / 2) : f / 2; }
+    __host__ __device__ static constexpr int hf(int f) { return NF == 5 ? (f == 0 ? 0 : f == 5 ? 1 : (f - 1) % 2) : f % 2; }
+};
+template <int NF>
+__device__ __forceinline__ float pget(const f2 *v, int f)
+{
+    return Pairs<NF>::hf(f) ? v[Pairs<NF>::pr(f)].y : v[Pairs<NF>::pr(f)].x;
+}
+template <int NF>
+__device__ __forceinline__ void pset(f2 *v, int f, float x)
+{
+    if (Pairs<NF>::hf(f)) v[Pairs<NF>::pr(f)].y = x; else v[Pairs<NF>::pr(f)].x = x;
+}
+
 template <int ORDER>
-__device__ __forceinline__ void recon(const float t[6], float &l, float &r)
+__device__ __forceinline__ void recon(const f2 t[6], f2 &l, f2 &r)
 {
     if (ORDER == 5) {
-        l = __fmul_rn(2.f / 60.f, t[0]);
-        l = __fmaf_rn(-13.f / 60.f, t[1], l);
-        l = __fmaf_rn(47.f / 60.f, t[2], l);
-        l = __fmaf_rn(27.f / 60.f, t[3], l);
-        l = __fmaf_rn(-3.f / 60.f, t[4], l);
-        r = __fmul_rn(-3.f / 60.f, t[1]);
-        r = __fmaf_rn(27.f / 60.f, t[2], r);
-        r = __fmaf_rn(47.f / 60.f, t[3], r);
-        r = __fmaf_rn(-13.f / 60.f, t[4], r);
-        r = __fmaf_rn(2.f / 60.f, t[5], r);
+        l = __fmul2_rn(splat(2.f / 60.f), t[0]);
+        l = __ffma2_rn(splat(-13.f / 60.f), t[1], l);
+        l = __ffma2_rn(splat(47.f / 60.f), t[2], l);
+        l = __ffma2_rn(splat(27.f / 60.f), t[3], l);
+        l = __ffma2_rn(splat(-3.f / 60.f), t[4], l);
+        r = __fmul2_rn(splat(-3.f / 60.f), t[1]);
+        r = __ffma2_rn(splat(27.f / 60.f), t[2], r);
+        r = __ffma2_rn(splat(47.f / 60.f), t[3], r);
+        r = __ffma2_rn(splat(-13.f / 60.f), t[4], r);
+        r = __ffma2_rn(splat(2.f / 60.f), t[5], r);
     } else {
-        l = __fmul_rn(-1.f / 6.f, t[1]);
-        l = __fmaf_rn(5.f / 6.f, t[2], l);
-        l = __fmaf_rn(2.f / 6.f, t[3], l);
-        r = __fmul_rn(2.f / 6.f, t[2]);
-        r = __fmaf_rn(5.f / 6.f, t[3], r);
-        r = __fmaf_rn(-1.f / 6.f, t[4], r);
+        l = __fmul2_rn(splat(-1.f / 6.f), t[1]);
+        l = __ffma2_rn(splat(5.f / 6.f), t[2], l);
+        l = __ffma2_rn(splat(2.f / 6.f), t[3], l);
+        r = __fmul2_rn(splat(2.f / 6.f), t[2]);
+        r = __ffma2_rn(splat(5.f / 6.f), t[3], r);
+        r = __ffma2_rn(splat(-1.f / 6.f), t[4], r);
     }
 }
 
@@ -149,21 +178,34 @@ __device__ __forceinline__ void side_flux2(const float *U, const Eos &eos, float
     F[IE] = __fmul_rn(__fadd_rn(U[IE], pt), ud);
 }
 
-// G = 2 F^ for the NF conserved fields; two fluids: G[NF] = u_d,L + u_d,R = 2 u^ (the face velocity of a1 div u)
+// G = 2 F^ for the NF conserved fields, in pairs (G[p] holds the components of the fields of pair p); two fluids:
+// the second half of the last pair is u_d,L + u_d,R = 2 u^ (the face velocity of a1 div u)
 template <int ORDER, int D, int NF>
-__device__ __forceinline__ void face_flux2(const float t[][6], float lam, const Eos &eos, float *G)
+__device__ __forceinline__ void face_flux2(const f2 t[][6], float lam, const Eos &eos, f2 *G)
 {
+    using PM = Pairs<NF>;
     constexpr int NC = NF == 5 ? 5 : NF + 1;
+    f2 L2[PM::NP], R2[PM::NP];
+#pragma unroll
+    for (int p = 0; p < PM::NP; ++p) recon<ORDER>(t[p], L2[p], R2[p]);
     float L[NF + 1], R[NF + 1];
 #pragma unroll
-    for (int f = 0; f < NF + 1; ++f) recon<ORDER>(t[f], L[f], R[f]);
+    for (int f = 0; f < NF + 1; ++f) { L[f] = pget<NF>(L2, f); R[f] = pget<NF>(R2, f); }
     float FL[NC], FR[NC];
     side_flux2<D, NF>(L, eos, FL);
     side_flux2<D, NF>(R, eos, FR);
 #pragma unroll
-    for (int c = 0; c < NF; ++c)
-        G[c] = __fmaf_rn(-lam, __fsub_rn(R[c], L[c]), __fadd_rn(FL[c], FR[c]));
-    if (NF != 5) G[NF] = __fadd_rn(FL[NF], FR[NF]);
+    for (int p = 0; p < PM::NP; ++p) {
+        if (NF == 5 && p == 2) {          // rho alone (Sigma has no flux)
+            G[p].x = __fmaf_rn(-lam, __fsub_rn(R[0], L[0]), __fadd_rn(FL[0], FR[0]));
+            G[p].y = 0.f;
+        } else {
+            const f2 fl = make_float2(FL[PM::fa(p)], FL[PM::fb(p)]), fr = make_float2(FR[PM::fa(p)], FR[PM::fb(p)]);
+            // (u^ carries no dissipation: its multiplier is zero)
+            const f2 nl = make_float2(-lam, (NF != 5 && p == PM::NP - 1) ? 0.f : -lam);
+            G[p] = __ffma2_rn(nl, fsub2(R2[p], L2[p]), __fadd2_rn(fl, fr));
+        }
+    }
 }
 
 // cell-centred wave speeds |u_d| + c of one cell (reading A5); explicit intrinsics as above.
@@ -200,7 +242,8 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 {
     using TL = Tile<T, TY, NF>;
     constexpr int NC = TL::NC;                                          // flux components per face
-    constexpr int NW = NF + 1;                                          // fields in the window: q and Sigma
+    using PM = Pairs<NF>;
+    constexpr int NP = PM::NP;                                          // pairs of fields in the window: q and Sigma
     constexpr bool TWO = NF != 5;
     extern __shared__ __align__(1024) unsigned char smem[];
     float *Abase = reinterpret_cast<float *>(smem + TL::A_OFF);         // [2][ax | ay][(TY+2)][AW]
@@ -243,21 +286,23 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     auto sbase = [&](int slot) { return reinterpret_cast<const T *>(smem + slot * TL::SLOT + TL::QBYTES); };
 
     // ---- prologue: window of planes p = 0..5 (cells kz0-3 .. kz0+2), flux of the face kz0-1/2
-    float W[NW][6];                                                // W[f][s]
+    f2 W[NP][6];                                                   // W[p][s]: pair p of the fields (struct Pairs)
 #pragma unroll
     for (int s = 0; s < 6; ++s) {
         mbar_wait(&full[s], 0);
-        const T *qb = qbase(s) + own;
+        const T *qb = qbase(s) + own, *sb = sbase(s) + own;
 #pragma unroll
-        for (int f = 0; f < NF; ++f) W[f][s] = lds<T>(qb + f * TL::PE);
-        W[NF][s] = lds<T>(sbase(s) + own);
+        for (int p = 0; p < NP; ++p) {
+            W[p][s].x = lds<T>(PM::fa(p) < NF ? qb + PM::fa(p) * TL::PE : sb);
+            W[p][s].y = lds<T>(PM::fb(p) < NF ? qb + PM::fb(p) * TL::PE : sb);
+        }
     }
     // the conserved values of the own column at window position s
     auto column = [&](int s, float *q) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) q[f] = W[f][s];
+        for (int f = 0; f < NF; ++f) q[f] = PM::hf(f) ? W[PM::pr(f)][s].y : W[PM::pr(f)][s].x;
     };
-    float Gz_prev[NC];
+    f2 Gz_prev[NP];
     float ax_c, ay_c, az_c;
     {
         float bx, by, az_m, q2[NF], q3[NF];
@@ -268,20 +313,22 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         (void)bx; (void)by;
     }
 #pragma unroll
-    for (int f = 0; f < NW; ++f) {
+    for (int p = 0; p < NP; ++p) {
 #pragma unroll
-        for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];          // now cells kz0-2 .. kz0+2 in W[.][0..4]
+        for (int s = 0; s < 5; ++s) W[p][s] = W[p][s + 1];          // now cells kz0-2 .. kz0+2 in W[.][0..4]
     }
     // cell-centred wave speeds |u_d| + c of plane p (own cells from registers, the halo ring of the
-    // tile from the ring slot, by warp 1) into the buffer of that plane's parity
+    // tile from the ring slot) into the buffer of that plane's parity
     auto put_speeds = [&](int p, int slot, float oax, float oay) {
         float *A0 = Abase + (p & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
         A0[(ty + 1) * TL::AW + tx + 1] = oax;
         A1[(ty + 1) * TL::AW + tx + 1] = oay;
-        if (warp == 1 % TY) {
+        // (warps 4, 5, 6 take 32 halo cells each: warps 2 and 3 have the edge faces, and the step ends at a barrier)
+        if (warp >= 4 && warp < 7) {
             // x-halo (tx = -1, 32) needs ax, y-halo (ty = -1, TY) needs ay
             const T *qp = qbase(slot);
-            for (int h = tx; h < 2 * TY + 2 * TX; h += 32) {
+            const int h = (warp - 4) * 32 + tx;
+            if (h < 2 * TY + 2 * TX) {
                 int hx, hy;
                 if (h < 2 * TY) { hx = (h & 1) ? TX : -1; hy = h >> 1; }
                 else { const int hh = h - 2 * TY; hy = (hh >= TX) ? TY : -1; hx = hh & (TX - 1); }
@@ -341,19 +388,21 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         const int slot_c1 = (slot_c == TL::NSLOT - 1) ? 0 : slot_c + 1;  // slot of plane pc + 1
         mbar_wait(&full[slot_n], phase_n);
         {
-            const T *qb = qbase(slot_n) + own;
+            const T *qb = qbase(slot_n) + own, *sb = sbase(slot_n) + own;
 #pragma unroll
-            for (int f = 0; f < NF; ++f) W[f][5] = lds<T>(qb + f * TL::PE);
-            W[NF][5] = lds<T>(sbase(slot_n) + own);
+            for (int p = 0; p < NP; ++p) {
+                W[p][5].x = lds<T>(PM::fa(p) < NF ? qb + PM::fa(p) * TL::PE : sb);
+                W[p][5].y = lds<T>(PM::fb(p) < NF ? qb + PM::fb(p) * TL::PE : sb);
+            }
         }
         // fused update: q^n of this cell is fetched now and consumed at the end of the step, so that
         // the global-load latency hides behind the flux computation
-        float qn_pre[NF];
+        f2 qn_pre[NP];
         const unsigned id = uid;                                    // element offset of cell (i, j, kz0 + t)
         uid += (unsigned)g.sz;
         if (FUSE && a.read_qn) {                                   // (columns beyond the domain read a valid
 #pragma unroll                                                      //  cell: the offset is clamped, nothing is stored)
-            for (int c = 0; c < NF; ++c) qn_pre[c] = ldf(reinterpret_cast<const T *>(a.qn[c]) + id);
+            for (int c = 0; c < NF; ++c) pset<NF>(qn_pre, c, ldf(reinterpret_cast<const T *>(a.qn[c]) + id));
         }
         // wave speeds of the next cell (k+1) of this column, published for the next step
         float ax_n, ay_n, az_n;
@@ -372,62 +421,47 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         float *FY = FYbase + (t & 1) * NC * TY * TX, *EX = EXbase + (t & 1) * NC * TY, *EY = EYbase + (t & 1) * NC * TX;
 
         const TC *sc = HALF ? qc + NF * TL::PE : reinterpret_cast<const TC *>(sbase(slot_c));
-        float Gx[NC], Gy[NC];
-        {   // x+ face of the own cell: cells i-2 .. i+3
-            float tp[NW][6];
-            const TC *qb = qc + own;
+        // the six taps of every field pair about a face: `at` = the box position of stencil cell 0, `st` = the tap stride
+        auto taps = [&](f2 tp[][6], int at, int st, bool own_col) {
 #pragma unroll
-            for (int f = 0; f < NF; ++f) {
+            for (int p = 0; p < NP; ++p) {
+                const TC *pa = (PM::fa(p) < NF ? qc + PM::fa(p) * TL::PE : sc) + at;
+                const TC *pb = (PM::fb(p) < NF ? qc + PM::fb(p) * TL::PE : sc) + at;
 #pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2));
+                for (int s = 0; s < 6; ++s) {
+                    if (own_col && s == 2) tp[p][s] = W[p][2];          // the own cell is in the window
+                    else { tp[p][s].x = lds<TC>(pa + s * st); tp[p][s].y = lds<TC>(pb + s * st); }
+                }
             }
-#pragma unroll
-            for (int s = 0; s < 6; ++s) tp[NF][s] = (s == 2) ? W[NF][2] : lds<TC>(sc + own + (s - 2));
+        };
+        f2 Gx[NP], Gy[NP];
+        {   // x+ face of the own cell: cells i-2 .. i+3
+            f2 tp[NP][6];
+            taps(tp, own - 2, 1, true);
             face_flux2<ORDER, 0, NF>(tp, fmaxf(ax_c, A0[(ty + 1) * TL::AW + tx + 2]), eos, Gx);
         }
         {   // y+ face: cells j-2 .. j+3
-            float tp[NW][6];
-            const TC *qb = qc + own;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-#pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = (s == 2) ? W[f][2] : lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
-            }
-#pragma unroll
-            for (int s = 0; s < 6; ++s) tp[NF][s] = (s == 2) ? W[NF][2] : lds<TC>(sc + own + (s - 2) * TL::BX);
+            f2 tp[NP][6];
+            taps(tp, own - 2 * TL::BX, TL::BX, true);
             face_flux2<ORDER, 1, NF>(tp, fmaxf(ay_c, A1[(ty + 2) * TL::AW + tx + 1]), eos, Gy);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) FY[(c * TY + ty) * TX + tx] = Gy[c];
+            for (int c = 0; c < NC; ++c) FY[(c * TY + ty) * TX + tx] = pget<NF>(Gy, c);
         }
         if (warp == 2 % TY && tx < TY) {
             // faces on the tile's low-x edge: between box columns HX-1 | HX of row tx
-            float tp[NW][6], Ge[NC];
-            const TC *qb = qc + (3 + tx) * TL::BX + TL::HX - 1;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-#pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2));
-            }
-#pragma unroll
-            for (int s = 0; s < 6; ++s) tp[NF][s] = lds<TC>(sc + (3 + tx) * TL::BX + TL::HX - 1 + (s - 2));
+            f2 tp[NP][6], Ge[NP];
+            taps(tp, (3 + tx) * TL::BX + TL::HX - 3, 1, false);
             face_flux2<ORDER, 0, NF>(tp, fmaxf(A0[(tx + 1) * TL::AW + 0], A0[(tx + 1) * TL::AW + 1]), eos, Ge);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) EX[c * TY + tx] = Ge[c];
+            for (int c = 0; c < NC; ++c) EX[c * TY + tx] = pget<NF>(Ge, c);
         }
         if (warp == 3 % TY) {
             // faces on the tile's low-y edge: between box rows 2 | 3 of column tx
-            float tp[NW][6], Ge[NC];
-            const TC *qb = qc + 2 * TL::BX + TL::HX + tx;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-#pragma unroll
-                for (int s = 0; s < 6; ++s) tp[f][s] = lds<TC>(qb + f * TL::PE + (s - 2) * TL::BX);
-            }
-#pragma unroll
-            for (int s = 0; s < 6; ++s) tp[NF][s] = lds<TC>(sc + 2 * TL::BX + TL::HX + tx + (s - 2) * TL::BX);
+            f2 tp[NP][6], Ge[NP];
+            taps(tp, TL::HX + tx, TL::BX, false);
             face_flux2<ORDER, 1, NF>(tp, fmaxf(A1[0 * TL::AW + tx + 1], A1[1 * TL::AW + tx + 1]), eos, Ge);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) EY[c * TX + tx] = Ge[c];
+            for (int c = 0; c < NC; ++c) EY[c * TX + tx] = pget<NF>(Ge, c);
         }
         __syncthreads();                                   // the only barrier of the step
         if (tid == 0 && t + 3 + TL::NSLOT < n_planes) {              // slot of plane pc is free again
@@ -436,34 +470,58 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         }
 
         // z+ face (cells k-2 .. k+3 of the own column), then the divergence
-        float Gz[NC];
+        f2 Gz[NP];
         face_flux2<ORDER, 2, NF>(W, fmaxf(az_c, az_n), eos, Gz);
-        float r[NC];
+        f2 r[NP];
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            float gxm = __shfl_up_sync(0xffffffffu, Gx[c], 1);
-            if (tx == 0) gxm = EX[c * TY + ty];
-            const float gym = (ty == 0) ? EY[c * TX + tx] : FY[(c * TY + ty - 1) * TX + tx];
+        for (int p = 0; p < NP; ++p) {
+            const int ca = PM::fa(p), cb = PM::fb(p);              // components of this pair (cb may be none)
+            f2 gxm, gym;
+            gxm.x = __shfl_up_sync(0xffffffffu, Gx[p].x, 1);
+            if (tx == 0) gxm.x = EX[ca * TY + ty];
+            gym.x = (ty == 0) ? EY[ca * TX + tx] : FY[(ca * TY + ty - 1) * TX + tx];
             // r = -(1/dx) sum_d (F^+ - F^-) with G = 2 F^
-            float acc = __fsub_rn(Gx[c], gxm);
-            acc = __fadd_rn(acc, __fsub_rn(Gy[c], gym));
-            acc = __fadd_rn(acc, __fsub_rn(Gz[c], Gz_prev[c]));
-            r[c] = __fmul_rn(-hdx, acc);
-            Gz_prev[c] = Gz[c];
+            if (cb < NC) {
+                gxm.y = __shfl_up_sync(0xffffffffu, Gx[p].y, 1);
+                if (tx == 0) gxm.y = EX[cb * TY + ty];
+                gym.y = (ty == 0) ? EY[cb * TX + tx] : FY[(cb * TY + ty - 1) * TX + tx];
+                f2 acc = fsub2(Gx[p], gxm);
+                acc = __fadd2_rn(acc, fsub2(Gy[p], gym));
+                acc = __fadd2_rn(acc, fsub2(Gz[p], Gz_prev[p]));
+                r[p] = __fmul2_rn(splat(-hdx), acc);
+            } else {
+                float acc = __fsub_rn(Gx[p].x, gxm.x);
+                acc = __fadd_rn(acc, __fsub_rn(Gy[p].x, gym.x));
+                acc = __fadd_rn(acc, __fsub_rn(Gz[p].x, Gz_prev[p].x));
+                r[p].x = __fmul_rn(-hdx, acc);
+                r[p].y = 0.f;
+            }
+            Gz_prev[p] = Gz[p];
         }
-        // two fluids: + a1 div u with the face velocities u^ (r[NF] = -(1/dx) sum_d (u^+ - u^-))
-        if (TWO) r[NF - 1] = __fmaf_rn(-W[NF - 1][2], r[NF], r[NF - 1]);
+        // two fluids: + a1 div u with the face velocities u^ (the last pair holds r of a1 and -(1/dx) sum_d (u^+ - u^-))
+        if (TWO) r[NP - 1].x = __fmaf_rn(-W[NP - 1][2].x, r[NP - 1].y, r[NP - 1].x);
         if (valid) {
             if (!FUSE) {
 #pragma unroll
-                for (int c = 0; c < NF; ++c) a.r[c][id] = r[c];
+                for (int c = 0; c < NF; ++c) a.r[c][id] = pget<NF>(r, c);
             } else {
+                f2 o2[NP];
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    const f2 qs = W[p][2];
+                    if (PM::fb(p) < NF) {
+                        const f2 qn = a.read_qn ? qn_pre[p] : qs;
+                        o2[p] = __ffma2_rn(splat(a.beta), __ffma2_rn(splat(a.dt), r[p], fsub2(qs, qn)), qn);
+                    } else {                                       // (x, Sigma): one field
+                        const float qn = a.read_qn ? qn_pre[p].x : qs.x;
+                        o2[p].x = __fmaf_rn(a.beta, __fmaf_rn(a.dt, r[p].x, __fsub_rn(qs.x, qn)), qn);
+                        o2[p].y = 0.f;
+                    }
+                }
                 float o[NF];
 #pragma unroll
                 for (int c = 0; c < NF; ++c) {
-                    const float qs = W[c][2];
-                    const float qn = a.read_qn ? qn_pre[c] : qs;
-                    o[c] = __fmaf_rn(a.beta, __fmaf_rn(a.dt, r[c], __fsub_rn(qs, qn)), qn);
+                    o[c] = pget<NF>(o2, c);
                     stf(reinterpret_cast<T *>(a.qout[c]) + id, o[c]);
                 }
                 if (a.wave && kz0 + t >= g.wk0 && kz0 + t < g.wk1) {
@@ -478,9 +536,9 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
         }
         // slide the window
 #pragma unroll
-        for (int f = 0; f < NW; ++f) {
+        for (int p = 0; p < NP; ++p) {
 #pragma unroll
-            for (int s = 0; s < 5; ++s) W[f][s] = W[f][s + 1];
+            for (int s = 0; s < 5; ++s) W[p][s] = W[p][s + 1];
         }
         ax_c = ax_n; ay_c = ay_n; az_c = az_n;
         slot_c = slot_c1;
