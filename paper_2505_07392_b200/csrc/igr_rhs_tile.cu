@@ -560,7 +560,10 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
 namespace {
 
 // two fluids: 168 registers per thread, one CTA per SM: 12 rows (384 threads) fill the register file
-constexpr int TY2 = 12;
+#ifndef IGR_RHS_TY2
+#define IGR_RHS_TY2 12
+#endif
+constexpr int TY2 = IGR_RHS_TY2;
 
 int tile_ty(const Grid &g)
 {
