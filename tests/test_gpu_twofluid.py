@@ -10,6 +10,7 @@ import pytest
 from paper_2505_07392_b200 import igr
 from paper_2505_07392_b200 import workloads as W
 import parity
+from test_gpu_configs import FULL, _subbox_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -34,6 +35,17 @@ def test_two_fluid_jets_three_steps_match_the_oracle(shape):
     assert l1 <= 1e-3 and mx <= 2e-3, (mx, l1, parity.norms(qg, qr))
     assert qr[1].min() > 0 and qr[0].min() > 0                     # both partial densities present everywhere
     assert np.ptp(qr[6]) > 0.9                                     # and a real interface
+
+
+@pytest.mark.skipif(not FULL, reason="full-size configs disabled")
+def test_two_fluid_jets33_1024_subbox_first_3_steps():
+    """The workload `bench.py --workload jets2f33_1024` times, in its launch configuration, against the two-fluid
+    oracle on the dependency-cone sub-box over the lip of an inner-ring jet (as for config 5 with one fluid)."""
+    w = W.two_fluid(W.jets33())
+    got, want, rho_min = _subbox_parity(w, (496, 480, 0), 64, 80, 3)
+    mx, l1 = parity.worst(got, want)
+    assert l1 <= 1e-3, (mx, l1, parity.norms(got, want))
+    assert rho_min > 0 and np.ptp(want[6]) > 0.9                    # an interface crosses the sub-box
 
 
 def test_two_fluid_interface_advection_keeps_u_and_p_uniform():
