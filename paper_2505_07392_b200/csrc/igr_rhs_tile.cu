@@ -18,7 +18,6 @@
 #include "igr_tma.cuh"
 
 #include <cstdio>
-#include <type_traits>
 #include <cstdlib>
 #include <cuda_fp16.h>
 #include <cuda_bf16.h>
@@ -26,8 +25,8 @@
 namespace {
 
 constexpr int TX = 32;          // tile width = warp width
-#ifndef IGR_RHS_NSLOT_HALF
-#define IGR_RHS_NSLOT_HALF 6
+#ifndef IGR_RHS_NSLOT2
+#define IGR_RHS_NSLOT2 6        // ring slots of the two-fluid kernel (8 fields per plane)
 #endif
 
 using namespace igr_tma;
@@ -47,7 +46,7 @@ __device__ __forceinline__ float sqrt_fast(float x)
 
 // ---- geometry of one ring slot for storage type T
 // NF = conserved fields (5: single fluid; 7: two fluids, reading A21)
-template <typename T, int TY, int NF = 5, int NSLOT_OF_T = (sizeof(T) == 4 && NF == 5 ? 7 : IGR_RHS_NSLOT_HALF)>
+template <typename T, int TY, int NF = 5, int NSLOT_OF_T = (NF == 5 ? 7 : IGR_RHS_NSLOT2)>
 struct Tile {
     static constexpr int NC = NF == 5 ? 5 : NF + 1;      // flux components exchanged per face (two fluids: + u^)
     static constexpr int NSLOT = NSLOT_OF_T;             // ring slots (planes): 4 live + 2 or 3 in flight
@@ -67,11 +66,7 @@ struct Tile {
     static constexpr int FY_OFF = A_OFF + 2 * 2 * A_N * 4;           // float [2][NC][TY][TX]
     static constexpr int EX_OFF = FY_OFF + 2 * NC * TY * TX * 4;     // float [2][NC][TY]
     static constexpr int EY_OFF = EX_OFF + 2 * NC * TY * 4;          // float [2][NC][TX]
-    // reduced-precision storage: the current plane is converted ONCE to fp32 (two buffers by plane
-    // parity, same box layout, Sigma after the five q fields) so that the stencil taps need no cvt
-    static constexpr int CUR_N = (sizeof(T) == 2) ? (NF + 1) * PE : 0; // floats per buffer
-    static constexpr int CUR_OFF = (EY_OFF + 2 * NC * TX * 4 + 15) / 16 * 16;
-    static constexpr int BAR_OFF = (CUR_OFF + 2 * CUR_N * 4 + 7) / 8 * 8;
+    static constexpr int BAR_OFF = (EY_OFF + 2 * NC * TX * 4 + 7) / 8 * 8;
     static constexpr int TOTAL = BAR_OFF + NSLOT * 8;
 };
 
@@ -250,8 +245,6 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
     float *FYbase = reinterpret_cast<float *>(smem + TL::FY_OFF);       // [2][NC][TY][TX]
     float *EXbase = reinterpret_cast<float *>(smem + TL::EX_OFF);       // [2][NC][TY]
     float *EYbase = reinterpret_cast<float *>(smem + TL::EY_OFF);       // [2][NC][TX]
-    float *CUR = reinterpret_cast<float *>(smem + TL::CUR_OFF);         // [2][NW][PE] (half storage only)
-    constexpr bool HALF = sizeof(T) == 2;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + TL::BAR_OFF);
 
     const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5, warp = ty;
@@ -342,29 +335,6 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             }
         }
     };
-    // half storage: plane p (ring slot `slot`) -> fp32 buffer of its parity, two elements per access
-    auto convert_plane = [&](int p, int slot) {
-        if (!HALF) return;
-        float2 *dq = reinterpret_cast<float2 *>(CUR + (p & 1) * TL::CUR_N);
-        const unsigned *sq = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT);
-        const unsigned *ss = reinterpret_cast<const unsigned *>(smem + slot * TL::SLOT + TL::QBYTES);
-        auto cv = [](unsigned v) {
-            if (std::is_same<T, __half>::value) return __half22float2(*reinterpret_cast<const __half2 *>(&v));
-            return __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&v));
-        };
-        constexpr int NT = TX * TY, NQ = NF * TL::PE / 2, NSG = TL::PE / 2;      // pairs of q / of Sigma
-#pragma unroll
-        for (int it = 0; it < (NQ + NT - 1) / NT; ++it) {
-            const int e = tid + it * NT;
-            if ((it + 1) * NT <= NQ || e < NQ) dq[e] = cv(sq[e]);
-        }
-#pragma unroll
-        for (int it = 0; it < (NSG + NT - 1) / NT; ++it) {
-            const int e = tid + it * NT;
-            if ((it + 1) * NT <= NSG || e < NSG) dq[NQ + e] = cv(ss[e]);
-        }
-    };
-    convert_plane(3, 3);
     put_speeds(3, 3, ax_c, ay_c);                                  // plane of the first cell layer kz0
     __syncthreads();                                               // planes 0..2 are no longer needed
     if (tid == 0) {
@@ -412,15 +382,14 @@ k_rhs_tile(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUt
             cell_speeds<NF>(q3, eos, ax_n, ay_n, az_n);
         }
         put_speeds(pc + 1, slot_c1, ax_n, ay_n);                  // read in the next step (after the barrier)
-        convert_plane(pc + 1, slot_c1);
-        // the current plane as seen by the stencil taps: the ring slot itself (fp32) or its fp32 copy
-        typedef typename std::conditional<HALF, float, T>::type TC;
-        const TC *qc = HALF ? reinterpret_cast<const TC *>(CUR + (pc & 1) * TL::CUR_N)
-                            : reinterpret_cast<const TC *>(qbase(slot_c));
+        // the current plane as seen by the stencil taps: the ring slot itself (2-byte storage: every tap is
+        // converted where it is read -- 66 conversions per cell, but no second pass through shared memory)
+        typedef T TC;
+        const TC *qc = qbase(slot_c);
         const float *A0 = Abase + (pc & 1) * 2 * TL::A_N, *A1 = A0 + TL::A_N;
         float *FY = FYbase + (t & 1) * NC * TY * TX, *EX = EXbase + (t & 1) * NC * TY, *EY = EYbase + (t & 1) * NC * TX;
 
-        const TC *sc = HALF ? qc + NF * TL::PE : reinterpret_cast<const TC *>(sbase(slot_c));
+        const TC *sc = sbase(slot_c);
         // the six taps of every field pair about a face: `at` = the box position of stencil cell 0, `st` = the tap stride
         auto taps = [&](f2 tp[][6], int at, int st, bool own_col) {
 #pragma unroll
