@@ -40,6 +40,9 @@ def parse():
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--row-power", type=float, default=0.0, metavar="SECONDS",
+                    help="N = 1: also loop every main row alone for SECONDS and report its time, board power and SM "
+                         "clock (`row_power`): which kernel runs into the power limit")
     ap.add_argument("--exchange", default="ipc", choices=["ipc", "sendrecv"],
                     help="N > 1: halo planes by CUDA IPC peer copies (falls back to sendrecv if IPC is refused) "
                          "or by torch.distributed send/recv")
@@ -78,7 +81,7 @@ class ClockSampler(threading.Thread):
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_power_cap,power.limit")
 
     def __init__(self, index):
         super().__init__(daemon=True)
@@ -102,8 +105,17 @@ class ClockSampler(threading.Thread):
         mx = [int(float(r[1])) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i] == "Active" for r in self.rows)]
+        def num(x):
+            try:
+                return float(x)
+            except ValueError:
+                return None
+        pw = sorted(v for v in (num(r[2]) for r in self.rows if len(r) > 2) if v is not None)
+        lim = [v for v in (num(r[7]) for r in self.rows if len(r) > 7) if v is not None]
+        # (power: the fp32 step sits at the board's limit, which is what pulls the SM clock below its maximum)
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+                "reasons": reasons, "samples": len(sm), "power_w": pw[len(pw) // 2] if pw else None,
+                "power_limit_w": max(lim) if lim else None}
 
 
 def measured_peaks():
@@ -408,6 +420,35 @@ def run_ours(args):
         e2e = {"value": job_numbers(t_e2e * 1e3, cells, world, w.nf)["grind_ns"], "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 8, "ms_per_step": t_e2e * 1e3, "pinned_host": pinned}
 
+    row_power = None
+    if args.row_power > 0 and world == 1 and not ss:
+        row_power = {}
+        load_initial()
+        g.halo_bc()
+        for name, fn in (("sigma_source", g.sigma_source), ("jacobi", g.jacobi), ("rhs", g.rhs), ("step", one_step)):
+            if name == "rhs" and w.nf != 5:
+                continue                                   # (the unfused RHS exists for one fluid only)
+            for _ in range(3):
+                fn()
+            g.sync()
+            smp = ClockSampler(local)
+            smp.start()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0, n = time.perf_counter(), 0
+            e0.record(g.stream)
+            while time.perf_counter() - t0 < args.row_power:
+                for _ in range(5):
+                    fn()
+                g.sync()
+                n += 5
+            e1.record(g.stream)
+            g.sync()
+            c = smp.stop()
+            row_power[name] = {"ms_per_call": e0.elapsed_time(e1) / n, "power_w": c["power_w"], "sm_mhz": c["sm_mhz"],
+                               "reasons": c["reasons"]}
+        row_power["note"] = ("each row looped alone; rhs = the unfused kernel (writes r, no q_n read); power_limit_w in "
+                             "`clocks`")
+
     out = {"metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.storage == "f64" else "f32",
@@ -424,6 +465,8 @@ def run_ours(args):
                       "resets": resets[0]},
            "cell_updates_per_s": job["cell_updates_per_s"],
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+    if row_power:
+        out["row_power"] = row_power
     if resets_timed[0]:
         # the state was reloaded inside the timed region (positivity lost, F1): the line is flagged
         out["invalid"] = "%d restart(s) from the initial state inside the timed region" % resets_timed[0]
