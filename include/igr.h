@@ -252,6 +252,30 @@ int igr_profile(igr_solver *s, int enable);    /* start (1) / stop (0) per-row C
                                                /* on the solver's stream; clears earlier records   */
 int igr_profile_read(igr_solver *s, double ms[6], long long count[6]); /* summed ms, calls per row */
 
+/* ---- the CFL wave speed without any allocation (igr_noalloc.cu).
+ * For callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it.  The same quantity as igr_max_wavespeed -- max over cells of max(|u|,|v|,|w|) + sqrt(gamma p / rho), Alg. 1
+ * L212-L215, readings A5/A9, same per-cell arithmetic -- but it needs no solver and calls no cudaMalloc, cudaFree or
+ * allocating library routine: the block partials of the reduction live in a file-scope device array of 512 KB that
+ * every GPU which loads the library holds until the process exits.
+ *   q       DEVICE pointer, fp32, the unpadded conserved fields [5][nz][ny][nx] (rho, mx, my, mz, E); borrowed,
+ *           read only.
+ *   out     DEVICE pointer to two floats, written by the call's last kernel: out[0] = the wave speed (the
+ *           maximum over the cells that gave a finite value), out[1] = 1 if any cell gave a non-finite value
+ *           (NaN/Inf, negative pressure or density: reported, not repaired, reading A10), else 0.
+ *   stream  a cudaStream_t (NULL: the default stream).  Two kernels are enqueued on it; the call does not wait
+ *           (the caller synchronises before reading `out` on the host) and is capturable after one warm call.
+ *   errbuf  optional host buffer of errbuf_len bytes for the message of a failure (may be NULL).
+ * Limit: nx * ny * nz <= IGR_NOALLOC_MAX_CELLS (2^30 = 1024^3; one slot of the array per 16384 cells); a larger
+ * state, a non-positive size, gamma <= 1 or a null pointer returns IGR_ERR_ARG and launches nothing.  The first
+ * call on a device (with that device current) resolves the array's device address (cudaGetSymbolAddress; checked).
+ * EVERY call on a device shares the array, which keeps the last call's contents: nothing in it must start at zero
+ * (each call overwrites every slot it reads), but two calls that overlap on the GPU -- different streams, or host
+ * threads on different streams -- RACE on it.  Order them on one stream or with events. */
+#define IGR_NOALLOC_MAX_CELLS (1LL << 30)
+int igr_max_wavespeed_noalloc(const float *q, int nx, int ny, int nz, double gamma, float *out, void *stream,
+                              char *errbuf, size_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,7 +28,9 @@ EXPORTS = ["igr_workspace_bytes", "igr_create", "igr_create_ex", "igr_destroy", 
            "igr_kernel_launches", "igr_profile", "igr_profile_read", "igr_set_viscosity", "igr_stage",
            "igr_export_fields", "igr_ipc_open", "igr_ipc_close", "igr_set_neighbor", "igr_pull_halo", "igr_set_wave_range", "igr_set_state_planes",
            "igr_get_state_planes", "igr_set_state_f64", "igr_get_state_f64", "igr_get_sigma_f64",
-           "igr_event_handle", "igr_event_open", "igr_event_close", "igr_event_record", "igr_event_wait"]
+           "igr_event_handle", "igr_event_open", "igr_event_close", "igr_event_record", "igr_event_wait",
+           "igr_max_wavespeed_noalloc"]
+NOALLOC_MAX_CELLS = 1 << 30      # igr.h IGR_NOALLOC_MAX_CELLS
 
 
 class IgrError(RuntimeError):
@@ -110,6 +112,7 @@ def lib():
         L.igr_event_wait.argtypes = [vp, vp]
         L.igr_last_error.argtypes = [vp]
         L.igr_last_error.restype = C.c_char_p
+        L.igr_max_wavespeed_noalloc.argtypes = [fp] + [C.c_int] * 3 + [C.c_double, fp, vp, C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
 
@@ -140,6 +143,26 @@ def _addr(a, shape, writable=False, f64=False):
     if writable:
         assert a.flags.writeable
     return a.ctypes.data
+
+
+def max_wavespeed_noalloc(q, gamma, out, stream=None, shape=None):
+    """igr_max_wavespeed_noalloc (igr.h): the CFL wave speed of the unpadded fp32 CUDA tensor q [5][nz][ny][nx] into
+    the 2-element fp32 CUDA tensor `out` (out[0] = speed, out[1] = non-finite flag), on `stream` (a raw cudaStream_t;
+    default: torch's current stream).  Nothing is allocated and nothing is waited for.  `shape` = (nz, ny, nx)
+    overrides q's own extents (the size check comes first: a refused size never touches q)."""
+    nz, ny, nx = (int(v) for v in (shape if shape is not None else q.shape[1:]))
+    if shape is None:
+        assert q.is_cuda and out.is_cuda
+        qa = _addr(q, (5, nz, ny, nx))
+    else:
+        qa = q.data_ptr()
+    oa = _addr(out, (2,), True)
+    if stream is None:
+        stream = torch.cuda.current_stream(out.device).cuda_stream
+    err = C.create_string_buffer(256)
+    rc = lib().igr_max_wavespeed_noalloc(qa, nx, ny, nz, float(gamma), oa, stream, err, len(err))
+    if rc != OK:
+        raise IgrError(rc, err.value.decode())
 
 
 def ipc_open(peer):
